@@ -1,0 +1,427 @@
+"""Pins of the CPU oracle (oracle/kgo.c) against things OTHER than itself: values the paper
+prints (tests/golden/paper_values.txt), closed forms, invariants, textbook results and dense
+exact diagonalisation (numpy.linalg) on lattices of <= 512 sites.  Chosen so that a plausible
+mistake in any oracle function (dropped term, wrong sign or index, transposed / unconjugated
+operand, wrong factor of 2, hbar or s) fails at least one test.  CPU only."""
+import numpy as np
+import pytest
+import scipy.special
+
+from helpers import HBAR, cheb_T, dense_h, golden, rand_state, relerr, ring
+
+T = -2.7
+A = 0.142
+S_GRAPHENE = 3 * 2.7 * 1.05
+
+
+def small_disordered(kgo, open_x=False):
+    """6x5 cells (120 sites) with 8 vacancies and Anderson disorder: no symmetry left."""
+    full = kgo.honeycomb(6, 5, periodic_x=not open_x, periodic_y=True)
+    vac = kgo.vacancy_mask(full.n, 8, 11)
+    lat = kgo.remove_sites(full, vac)
+    lat.onsite = kgo.anderson(lat.n, 2.7, 5)
+    return lat
+
+
+def eig(lat):
+    H = dense_h(lat)
+    assert np.allclose(H, H.T)
+    E, Vec = np.linalg.eigh(H)
+    return H, E, Vec
+
+
+def dense_U(E, Vec, dt):
+    """exp(-i H dt / hbar) from the eigen-decomposition."""
+    return (Vec * np.exp(-1j * E * dt / HBAR)) @ Vec.conj().T
+
+
+def dense_Tn(E, Vec, n, e0, s):
+    return (Vec * cheb_T(n, (E - e0) / s)) @ Vec.T
+
+
+# ------------------------------------------------------------------ H apply / moments (O2, O3)
+def test_apply_h_matches_dense(kgo):
+    lat = small_disordered(kgo)
+    H = dense_h(lat)
+    phi = rand_state(lat.n, 0)
+    e0, s = 0.3, 11.0
+    want = (H @ phi - e0 * phi) / s
+    assert relerr(kgo.apply_h(lat, e0, s, phi), want) < 1e-14
+
+
+def test_mu0_is_one_and_mu1_is_expectation(kgo):
+    lat = small_disordered(kgo)
+    H = dense_h(lat)
+    phi = rand_state(lat.n, 1)
+    mu = kgo.dos_moments(lat, 0.0, 10.0, phi, 4)
+    assert abs(mu[0] - 1.0) < 1e-14                       # normalised trace: mu_0 = 1
+    assert abs(mu[1] - np.vdot(phi, H @ phi) / 10.0) < 1e-14
+    assert np.max(np.abs(mu.imag)) < 1e-15                # <phi|T_n(H)|phi> is real
+
+
+def test_full_trace_closed_forms_pristine(kgo):
+    """Tr[T_2(H~)]/N = 2 z t^2/s^2 - 1 (z = 3); odd full-trace moments vanish on the bipartite
+    lattice with no on-site terms (BASELINE north_star; reading g20: full trace)."""
+    lat = kgo.honeycomb(4, 4)
+    n, M = lat.n, 8
+    tr = np.zeros(M, complex)
+    for j in range(n):
+        e = np.zeros(n, complex); e[j] = 1.0
+        tr += kgo.dos_moments(lat, 0.0, S_GRAPHENE, e, M)
+    tr /= n
+    assert abs(tr[0] - 1.0) < 1e-15
+    assert abs(tr[2] - (2 * 3 * T**2 / S_GRAPHENE**2 - 1)) < 1e-14
+    assert abs(tr[2] - (-0.395313681028)) < 1e-11
+    assert np.max(np.abs(tr[1::2])) < 1e-15
+    # one-sublattice vector: odd moments exactly zero per vector
+    phi = rand_state(n, 3); phi[1::2] = 0; phi /= np.linalg.norm(phi)
+    mu = kgo.dos_moments(lat, 0.0, S_GRAPHENE, phi, M)
+    assert np.max(np.abs(mu[1::2])) < 1e-16
+
+
+def test_ring_trace_closed_form(kgo):
+    """1-D ring, s = 2|t|: eigenvalues -cos(2 pi j/N) => Tr[T_n]/N = (-1)^n [N | n]."""
+    n, M = 12, 30
+    lat = ring(kgo, n)
+    tr = np.zeros(M, complex)
+    for j in range(n):
+        e = np.zeros(n, complex); e[j] = 1.0
+        tr += kgo.dos_moments(lat, 0.0, 2 * 2.7, e, M)
+    tr /= n
+    want = np.array([(-1.0) ** m if m % n == 0 else 0.0 for m in range(M)])
+    assert np.max(np.abs(tr - want)) < 1e-13
+
+
+def test_moments_vs_dense_diagonalisation(kgo):
+    """mu_n = sum_j conj(<j|phi_L>) <j|phi_R> T_n((E_j-E0)/s) — pins the recursion, the
+    scaling/shift, and the conjugation of the LEFT vector."""
+    lat = small_disordered(kgo)
+    _, E, Vec = eig(lat)
+    e0, s = 0.2, (3 * 2.7 + 1.35 + 0.2) * 1.05
+    assert np.max(np.abs(E - e0)) < s
+    phiL, phiR = rand_state(lat.n, 4), rand_state(lat.n, 5)
+    cL, cR = Vec.T @ phiL, Vec.T @ phiR
+    M = 200
+    want = np.array([np.sum(np.conj(cL) * cR * cheb_T(m, (E - e0) / s)) for m in range(M)])
+    got = kgo.moments(lat, e0, s, phiL, phiR, M)
+    assert relerr(got, want) < 1e-12
+    got_dos = kgo.dos_moments(lat, e0, s, phiR, M)
+    want_dos = np.array([np.sum(np.abs(cR) ** 2 * cheb_T(m, (E - e0) / s)) for m in range(M)])
+    assert relerr(got_dos, want_dos) < 1e-12
+
+
+# ------------------------------------------------------------------ Bessel (R4)
+def test_bessel_truncation_matches_paper(kgo):
+    val, tol = golden("np_at_pi")                          # "about 20" at argument pi, 1e-15
+    eps = golden("bessel_accuracy")[0]
+    np_pi = kgo.bessel_np(np.pi, eps)
+    assert abs(np_pi - val) <= tol and np_pi == 21
+    # the terms kept really are all those >= eps, scanning from above (reading g6)
+    for x in (0.3, np.pi, 6.3, 14.7, 25.2, 80.0):
+        n_p = kgo.bessel_np(x, eps)
+        jv = scipy.special.jv(np.arange(n_p + 40), x)
+        assert abs(jv[n_p - 1]) >= eps and np.all(np.abs(jv[n_p:]) < eps)
+    assert abs(20 / np.pi - golden("kpm_vs_ftm_cost")[0]) < golden("kpm_vs_ftm_cost")[1]
+
+
+def test_bessel_values(kgo):
+    for x in (0.3, np.pi, 6.3, 14.7, 25.2):
+        n_p = kgo.bessel_np(x)
+        j = kgo.bessel_j(x, n_p)
+        assert abs(j[0] ** 2 + 2 * np.sum(j[1:] ** 2) - 1.0) < 2e-15      # sum rule
+        assert np.max(np.abs(j - scipy.special.jv(np.arange(n_p), x))) < 2e-15
+
+
+# ------------------------------------------------------------------ evolution (O4)
+@pytest.mark.parametrize("e0", [0.0, 0.4])
+def test_evolve_vs_dense_expm(kgo, e0):
+    lat = small_disordered(kgo)
+    _, E, Vec = eig(lat)
+    s = (3 * 2.7 + 1.35 + 0.4) * 1.05
+    phi = rand_state(lat.n, 6)
+    for dt in (0.25, -0.25, 1.7, -1.7):
+        want = dense_U(E, Vec, dt) @ phi
+        got = kgo.evolve(lat, e0, s, phi, dt)
+        assert relerr(got, want) < 1e-12
+
+
+def test_evolve_unitarity_and_reversibility(kgo):
+    lat = small_disordered(kgo)
+    s = (3 * 2.7 + 1.35) * 1.05
+    phi = rand_state(lat.n, 7)
+    dt = 4 * HBAR / 2.7
+    psi = kgo.evolve(lat, 0.0, s, phi, dt)
+    assert abs(np.linalg.norm(psi) - 1.0) < 1e-12                 # |U phi| = |phi| to 1e-12
+    back = kgo.evolve(lat, 0.0, s, psi, -dt)
+    assert np.max(np.abs(back - phi)) < 1e-12                     # U(-dt) U(dt) phi = phi
+    assert np.max(np.abs(psi - phi)) > 0.1                        # and it did something
+
+
+def test_infinite_chain_amplitude(kgo):
+    """|<j|U(t)|0>| = |J_j(2|t| t/hbar)| on a chain long enough that wrap-around is negligible."""
+    n = 400
+    lat = ring(kgo, n)
+    e = np.zeros(n, complex); e[0] = 1.0
+    tt = 3.0
+    psi = kgo.evolve(lat, 0.0, 2 * 2.7 * 1.05, e, tt)
+    j = np.minimum(np.arange(n), n - np.arange(n))
+    want = np.abs(scipy.special.jv(j, 2 * 2.7 * tt / HBAR))
+    assert np.max(np.abs(np.abs(psi) - want)) < 1e-13
+
+
+# ------------------------------------------------------------------ velocity (O2, a5)
+def test_velocity_open_boundary_dense_commutator(kgo):
+    """V = (i/hbar)[H, X] as dense matrices when X is single-valued (open along x)."""
+    lat = small_disordered(kgo, open_x=True)
+    H = dense_h(lat)
+    X = np.diag(lat.x)
+    V = (1j / HBAR) * (H @ X - X @ H)
+    phi = rand_state(lat.n, 8)
+    got = kgo.apply_velocity(lat, lat.x, 0.0, phi)
+    assert relerr(got, V @ phi) < 1e-14
+    # [X, H~]
+    s = 9.7
+    got = kgo.apply_xh(lat, lat.x, 0.0, s, phi)
+    assert relerr(got, (X @ H - H @ X) @ phi / s) < 1e-14
+
+
+def test_velocity_hermitian_and_trace(kgo):
+    """<a|Vb> = <Va|b>; pristine Tr[V^2]/N = (3/2)(t a/hbar)^2 for either axis."""
+    lat = kgo.honeycomb(4, 4)
+    a, b = rand_state(lat.n, 9), rand_state(lat.n, 10)
+    for xc, per in ((lat.x, lat.period_x), (lat.y, lat.period_y)):
+        lhs = np.vdot(a, kgo.apply_velocity(lat, xc, per, b))
+        rhs = np.vdot(kgo.apply_velocity(lat, xc, per, a), b)
+        assert abs(lhs - rhs) < 1e-14
+        tr = 0.0
+        for j in range(lat.n):
+            e = np.zeros(lat.n, complex); e[j] = 1.0
+            tr += np.linalg.norm(kgo.apply_velocity(lat, xc, per, e)) ** 2
+        assert abs(tr / lat.n - 1.5 * (T * A / HBAR) ** 2) < 1e-13
+        assert abs(tr / lat.n - 0.508937) < 1e-6
+
+
+def test_velocity_group_velocity_on_ring(kgo):
+    """Plane wave on a periodic ring: V|k> = (1/hbar) dE/dk |k>, E = 2t cos(ka) — pins the sign
+    and the minimum-image convention across the periodic boundary (reading g2)."""
+    n = 16
+    lat = ring(kgo, n)
+    for jk in (1, 3, 5, 11):
+        k = 2 * np.pi * jk / (n * A)
+        pw = np.exp(1j * k * lat.x) / np.sqrt(n)
+        vg = -2 * T * A * np.sin(k * A) / HBAR
+        got = kgo.apply_velocity(lat, lat.x, lat.period_x, pw)
+        assert np.max(np.abs(got - vg * pw)) < 1e-14
+
+
+# ------------------------------------------------------------------ commutator evolution (O5)
+@pytest.mark.parametrize("e0", [0.0, -0.3])
+def test_comm_evolve_open_boundary_dense(kgo, e0):
+    """[X, U(dt)] = X U - U X with the dense U (open along x)."""
+    lat = small_disordered(kgo, open_x=True)
+    _, E, Vec = eig(lat)
+    s = (3 * 2.7 + 1.35 + 0.3) * 1.05
+    X = np.diag(lat.x)
+    phi = rand_state(lat.n, 12)
+    for dt in (0.3, 2.1):
+        U = dense_U(E, Vec, dt)
+        want = (X @ U - U @ X) @ phi
+        got = kgo.comm_evolve(lat, lat.x, 0.0, e0, s, phi, dt)
+        assert relerr(got, want) < 1e-12
+
+
+def test_comm_evolve_periodic_eigenbasis(kgo):
+    """Under PBC: <a|[X,U(t)]|b> = <a|[X,H]|b> (e^{-iE_b t} - e^{-iE_a t})/(E_b - E_a) in the
+    eigenbasis (degenerate pairs -> -(it/hbar) e^{-iE_a t/hbar}), with [X,H] the bond operator."""
+    lat = small_disordered(kgo, open_x=False)
+    H, E, Vec = eig(lat)
+    n = lat.n
+    # bond operator [X,H]_{im} = (x_i - x_m)_minimg H_im built from the dense H and coordinates
+    dx = lat.x[:, None] - lat.x[None, :]
+    dx -= lat.period_x * np.round(dx / lat.period_x)
+    XH = dx * (H - np.diag(np.diag(H)))
+    XHe = Vec.T @ XH @ Vec
+    dt = 1.3
+    ph = np.exp(-1j * E * dt / HBAR)
+    dE = E[None, :] - E[:, None]                         # E_b - E_a, index [a, b]
+    with np.errstate(divide="ignore", invalid="ignore"):
+        F = (ph[None, :] - ph[:, None]) / dE
+    deg = np.abs(dE) < 1e-9
+    F[deg] = (-1j * dt / HBAR) * np.broadcast_to(ph[:, None], (n, n))[deg]
+    XU = Vec @ (XHe * F) @ Vec.T
+    phi = rand_state(n, 13)
+    s = (3 * 2.7 + 1.35) * 1.05
+    got = kgo.comm_evolve(lat, lat.x, lat.period_x, 0.0, s, phi, dt)
+    assert relerr(got, XU @ phi) < 1e-11
+
+
+def test_comm_evolve_plane_wave_ring(kgo):
+    """Ring: [X,U(t)]|k> = (t/hbar) E'(k) e^{-iE_k t/hbar}|k>."""
+    n = 20
+    lat = ring(kgo, n)
+    tt = 0.9
+    for jk in (2, 7):
+        k = 2 * np.pi * jk / (n * A)
+        pw = np.exp(1j * k * lat.x) / np.sqrt(n)
+        Ek = 2 * T * np.cos(k * A)
+        dEk = -2 * T * A * np.sin(k * A)
+        want = (tt / HBAR) * dEk * np.exp(-1j * Ek * tt / HBAR) * pw
+        got = kgo.comm_evolve(lat, lat.x, lat.period_x, 0.0, 2 * 2.7 * 1.05, pw, tt)
+        assert np.max(np.abs(got - want)) < 1e-13
+
+
+# ------------------------------------------------------------------ VAC / MSD drivers (O7, O8)
+def test_vac_vs_dense(kgo):
+    """mu^VAC_n(t_k) = <V U^dag(t_k) phi | T_n(H~) | U^dag(t_k) V phi>  (eq 33)."""
+    lat = small_disordered(kgo, open_x=True)
+    H, E, Vec = eig(lat)
+    s = (3 * 2.7 + 1.35) * 1.05
+    X = np.diag(lat.x)
+    V = (1j / HBAR) * (H @ X - X @ H)
+    phi = rand_state(lat.n, 14)
+    M, nt, dt = 24, 3, 0.7
+    got = kgo.vac(lat, lat.x, 0.0, 0.0, s, phi, M, nt, dt)
+    assert got.shape == (nt + 1, M)
+    want = np.empty_like(got)
+    for k in range(nt + 1):
+        Ud = dense_U(E, Vec, -k * dt)
+        L = V @ (Ud @ phi)
+        R = Ud @ (V @ phi)
+        for m in range(M):
+            want[k, m] = np.vdot(L, dense_Tn(E, Vec, m, 0.0, s) @ R)
+    assert relerr(got, want) < 1e-12
+    # row 0 equals moments(V phi, V phi)
+    vphi = kgo.apply_velocity(lat, lat.x, 0.0, phi)
+    assert relerr(got[0], kgo.moments(lat, 0.0, s, vphi, vphi, M)) < 1e-15
+
+
+def test_msd_vs_dense(kgo):
+    """mu^MSD_n(t_k) = <psix_k|T_n(H~)|psix_k>, psix_k = [X, U(t_k)] phi = (X U^k - U^k X) phi
+    (eq 34; eq 44 composition)."""
+    lat = small_disordered(kgo, open_x=True)
+    _, E, Vec = eig(lat)
+    s = (3 * 2.7 + 1.35) * 1.05
+    X = np.diag(lat.x)
+    phi = rand_state(lat.n, 15)
+    M, nt, dt = 24, 3, 0.7
+    got = kgo.msd(lat, lat.x, 0.0, 0.0, s, phi, M, nt, dt)
+    want = np.empty_like(got)
+    for k in range(nt + 1):
+        U = dense_U(E, Vec, k * dt)
+        px = (X @ U - U @ X) @ phi
+        for m in range(M):
+            want[k, m] = np.vdot(px, dense_Tn(E, Vec, m, 0.0, s) @ px)
+    assert np.all(got[0] == 0)                                        # row 0 is exactly 0
+    assert relerr(got, want) < 1e-12
+    assert np.max(np.abs(got.imag)) < 1e-12 * np.max(np.abs(got))
+
+
+def test_ring_vac_constant_msd_quadratic(kgo):
+    """1-D ring: [V,H] = 0 => mu^VAC_n(t) independent of t and mu^MSD_n(t) = t^2 <V phi|T_n|V phi>
+    per vector, exactly."""
+    n = 64
+    lat = ring(kgo, n)
+    s = 2 * 2.7 * 1.05
+    phi = rand_state(n, 16)
+    M, nt, dt = 16, 4, 0.5
+    v = kgo.vac(lat, lat.x, lat.period_x, 0.0, s, phi, M, nt, dt)
+    m = kgo.msd(lat, lat.x, lat.period_x, 0.0, s, phi, M, nt, dt)
+    vphi = kgo.apply_velocity(lat, lat.x, lat.period_x, phi)
+    base = kgo.moments(lat, 0.0, s, vphi, vphi, M)
+    for k in range(nt + 1):
+        assert relerr(v[k], base) < 1e-12
+        assert np.max(np.abs(m[k] - (k * dt) ** 2 * base)) < 1e-12 * max(1.0, (k * dt) ** 2) * np.max(np.abs(base))
+
+
+def test_msd_small_time_limit(kgo):
+    """mu^MSD_0(t) = |psix|^2 -> <phi|V^2|phi> t^2 as t -> 0."""
+    lat = kgo.honeycomb(4, 4)
+    phi = rand_state(lat.n, 17)
+    dt = 1e-3
+    m = kgo.msd(lat, lat.x, lat.period_x, 0.0, S_GRAPHENE, phi, 2, 1, dt)
+    v2 = np.linalg.norm(kgo.apply_velocity(lat, lat.x, lat.period_x, phi)) ** 2
+    assert abs(m[1, 0].real / dt**2 - v2) < 1e-4 * v2
+
+
+# ------------------------------------------------------------------ reconstruction (O9)
+def test_reconstruct_single_moments(kgo):
+    """mu = delta_{n0} -> 1/(pi s sqrt(1-E~^2)); mu = delta_{n1} -> 2 g_1 E~ /(pi s sqrt(1-E~^2)):
+    pins the prefactor, the (2 - delta_n0) factor and T_n; g_0 = 1."""
+    M, s, e0 = 16, 8.5, 0.1
+    en = np.linspace(-7, 7, 29)
+    et = (en - e0) / s
+    g = kgo.jackson(M)
+    assert abs(g[0] - 1.0) < 1e-15
+    mu = np.zeros(M, complex); mu[0] = 1
+    assert relerr(kgo.kpm_reconstruct(mu, e0, s, en), 1 / (np.pi * s * np.sqrt(1 - et**2))) < 1e-14
+    mu = np.zeros(M, complex); mu[1] = 1
+    assert relerr(kgo.kpm_reconstruct(mu, e0, s, en), 2 * g[1] * et / (np.pi * s * np.sqrt(1 - et**2))) < 1e-14
+    mu = np.zeros(M, complex); mu[5] = 1j                       # only Re mu enters (reading g12)
+    assert np.max(np.abs(kgo.kpm_reconstruct(mu, e0, s, en))) == 0.0
+
+
+def test_jackson_kernel_positive_normalised_narrow(kgo):
+    """Jackson-damped delta: positive everywhere, integrates to 1, width ~ pi s/M; the undamped
+    (Dirichlet) kernel is not positive — a wrong alpha or a dropped term breaks positivity."""
+    M, s = 64, 1.0
+    y = 0.3
+    mu = cheb_T(np.arange(M), y).astype(complex)
+    # Chebyshev-Gauss nodes: integral f dE = (pi/K) sum sqrt(1-x_k^2) f(x_k)
+    K = 4096
+    xk = np.cos(np.pi * (np.arange(K) + 0.5) / K)
+    f = kgo.kpm_reconstruct(mu, 0.0, s, xk)
+    w = np.pi / K * np.sqrt(1 - xk**2)
+    assert f.min() > -1e-12
+    assert abs(np.sum(w * f) - 1.0) < 1e-12
+    mean = np.sum(w * f * xk)
+    sig = np.sqrt(np.sum(w * f * (xk - mean) ** 2))
+    assert 0.8 < sig / (np.pi / M * np.sqrt(1 - y**2)) < 1.2
+    f_raw = kgo.kpm_reconstruct(mu, 0.0, s, xk, use_jackson=False)
+    assert f_raw.min() < -0.1
+    g = kgo.jackson(M)
+    assert np.all(np.diff(g) < 0) and 0 < g[-1] < 0.01
+
+
+def graphene_dos_closed_form(E, t=2.7):
+    """Hobson-Nierenberg closed form, per site (integrates to 1): rho(E) =
+    (1/pi^2)(|E|/t^2) K(Z1/Z0)/sqrt(Z0), Z0=(1+e)^2-(e^2-1)^2/4, Z1=4e for e=|E/t|<=1, swapped for
+    1<=e<=3; K = complete elliptic integral with PARAMETER m (scipy convention)."""
+    e = np.abs(E) / t
+    z0 = (1 + e) ** 2 - (e**2 - 1) ** 2 / 4
+    z1 = 4 * e
+    lo = e <= 1
+    Z0 = np.where(lo, z0, z1)
+    Z1 = np.where(lo, z1, z0)
+    out = (1 / np.pi**2) * (np.abs(E) / t**2) * scipy.special.ellipk(Z1 / Z0) / np.sqrt(Z0)
+    return np.where(e < 3, out, 0.0)
+
+
+def test_pristine_graphene_dos_closed_form(kgo):
+    """DOS from oracle moments of random-phase vectors on a 48x48-cell sheet against the
+    closed form, away from the van Hove points |E| = |t| and from E = 0 / band edges, within the
+    Jackson width pi s/M and the stochastic error ~ 1/sqrt(N)."""
+    lat = kgo.honeycomb(48, 48)
+    n = lat.n
+    M, nvec = 96, 6
+    mu = np.zeros(M, complex)
+    for r in range(nvec):                                       # average of 6 random-phase vectors
+        u = kgo.phase_uniforms(n, 0, r)
+        phi = np.exp(2j * np.pi * u) / np.sqrt(n)
+        mu_r = kgo.dos_moments(lat, 0.0, S_GRAPHENE, phi, M)
+        assert abs(mu_r[0] - 1) < 1e-13
+        assert np.max(np.abs(mu_r[1::2])) < 6 / np.sqrt(n)      # statistical, reading g20
+        mu += mu_r / nvec
+    en = np.concatenate([np.linspace(-7.0, -3.6, 12), np.linspace(-1.9, -0.9, 8),
+                         np.linspace(0.9, 1.9, 8), np.linspace(3.6, 7.0, 12)])
+    rho = kgo.kpm_reconstruct(mu, 0.0, S_GRAPHENE, en)
+    ref = graphene_dos_closed_form(en)
+    # closed form integrates to 1 (checks the fixture itself)
+    g = np.linspace(-8.1, 8.1, 200001)
+    assert abs(np.trapezoid(graphene_dos_closed_form(g), g) - 1.0) < 2e-3
+    assert np.max(np.abs(rho - ref) / ref) < 0.12
+    assert abs(np.mean((rho - ref) / ref)) < 0.03
+    # integral of the reconstructed DOS is mu_0 = 1
+    K = 2048
+    xk = np.cos(np.pi * (np.arange(K) + 0.5) / K)
+    f = kgo.kpm_reconstruct(mu, 0.0, S_GRAPHENE, xk * S_GRAPHENE)
+    assert abs(np.sum(np.pi / K * np.sqrt(1 - xk**2) * f) * S_GRAPHENE - 1.0) < 1e-12
