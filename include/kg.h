@@ -1,0 +1,189 @@
+/*
+ * kg.h — C ABI of libkg: the Chebyshev hot path of the linear-scaling real-space
+ * Kubo-Greenwood method (arXiv 1307.0288), hand-written CUDA for NVIDIA B200 (sm_100a).
+ *
+ * "P:n" cites line n of PAPER.md (the paper's text).  Notation follows the paper:
+ *   H      sparse real-symmetric tight-binding Hamiltonian given as a neighbour list
+ *          NN_n / NL_nk with matrix elements H_{n,NL_nk}               (Alg. 8)
+ *   X      diagonal position operator, X_m                                     (eq 14)
+ *   V      velocity (i/hbar)[H, X]                                             (eq 15)
+ *   H~     (H - E0)/s, spectrum inside [-1, 1]
+ *   T_m    Chebyshev polynomials, T_m = 2 H~ T_{m-1} - T_{m-2}                 (eq 38)
+ *   U(dt)  exp(-i H dt/hbar) = sum_m (2-d_m0)(-i)^m J_m(s dt/hbar) T_m(H~)     (eq 36)
+ *
+ * Units: eV, nm, fs; hbar = 0.6582119569 eV fs.
+ *
+ * POINTERS.  Every array argument may be a DEVICE pointer (cudaMalloc / torch CUDA tensor)
+ * or a HOST pointer (pageable or pinned); the library detects which with
+ * cudaPointerGetAttributes.  Host inputs are copied to library-owned device staging
+ * buffers on `stream`; host outputs are written by an asynchronous device->host copy on
+ * `stream` (for pageable memory CUDA makes that copy synchronous).  All arithmetic runs in
+ * CUDA kernels; there is no CPU fallback.  All arrays are caller-owned and only borrowed for
+ * the duration of the call; inputs are never modified; `out` must not alias `in`.
+ *
+ * VECTORS are `[n][R]` complex128, site-major (the R values of one site are contiguous,
+ * element (site i, vector r) at index i*R + r), R in {1, 2, 4, 8} (kg_evolve and
+ * kg_apply_velocity also accept 16).  kg_c128 is layout-compatible with C99 `double complex`,
+ * std::complex<double> and torch.complex128.
+ *
+ * STREAMS.  `stream` is a cudaStream_t cast to void* (NULL = legacy default stream).  Calls
+ * enqueue work on it and return without synchronising, except kg_create_hamiltonian (which
+ * validates and therefore synchronises) and calls whose outputs are pageable host memory.
+ * Device outputs are valid once the stream has been synchronised.
+ *
+ * ERRORS.  Every call returns KG_OK or an error code; nothing throws or aborts across the
+ * ABI.  kg_last_error() returns a thread-local description of the last failure.
+ *
+ * A handle owns its device copy of the matrix and a lazily grown workspace (Chebyshev
+ * vectors T_m, accumulators, per-block moment partials).  A handle is not thread-safe.
+ */
+#ifndef KG_H
+#define KG_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct kg_hamiltonian kg_hamiltonian; /* opaque, library-owned */
+typedef struct { double re, im; } kg_c128;
+
+enum {
+    KG_OK = 0,
+    KG_EINVAL = 1,       /* null pointer, bad size, index out of range, non-finite value, aliasing */
+    KG_ENOMEM = 2,       /* device allocation failed */
+    KG_ECUDA = 3,        /* CUDA runtime error (text in kg_last_error) */
+    KG_ESPECTRUM = 4,    /* Gershgorin bound of (H - E0) exceeds s: recursion would diverge */
+    KG_EUNSUPPORTED = 5  /* R not in the supported set, kmax too large */
+};
+
+/* Thread-local message of the last error returned on this thread ("" if none). */
+const char *kg_last_error(void);
+
+/*
+ * kg_create_hamiltonian — build the scaled operator H~ = (H - E0)/s and the commutator
+ * weights of [X, H~] from the paper's neighbour list (Alg. 8 "Require" lines
+ * P:420-425; scaling P:192; [X,H] eq 15, eq 41).
+ *
+ *   n          number of sites (1 <= n < 2^31)
+ *   kmax       row width of the list (1 <= kmax <= 32)
+ *   nn[n]      NN_i, number of neighbours of site i (0 <= nn[i] <= kmax)
+ *   nl[kmax*n] NL_ik at nl[k*n + i]  — k-major, "NL_00, NL_10, NL_20, ..., NL_01, ...";
+ *              entries with k >= nn[i] are ignored
+ *   hop_eV     H_{i,NL_ik} at hop_eV[k*n + i], real (eq 13), eV
+ *   onsite_eV  H_ii, eV; NULL = 0
+ *   x_nm[n]    X_i, the coordinate along the transport direction, nm
+ *   period_x_nm  period of that coordinate; <= 0: open boundary.  Bond displacements
+ *              X_m - X_i are reduced to the minimum image when periodic.
+ *   e0_eV, scale_eV   H~ = (H - e0)/scale, scale > 0 (the half-width "Delta E" of
+ *              BASELINE.json; NOT the paper's full bandwidth of eq 47-49)
+ *
+ * Validates (indices in range, counts <= kmax, finite values, H symmetric, Gershgorin bound
+ * max_i(|H_ii - E0| + sum_k |H_ik|) <= s) on the device, synchronises `stream`, and returns
+ * KG_EINVAL / KG_ESPECTRUM accordingly.  The caller may free its arrays after the call.
+ */
+int kg_create_hamiltonian(kg_hamiltonian **out, int64_t n, int32_t kmax, const int32_t *nn,
+                          const int32_t *nl, const double *hop_eV, const double *onsite_eV,
+                          const double *x_nm, double period_x_nm, double e0_eV, double scale_eV,
+                          void *stream);
+
+/* Same operator from CSR: rowptr[n+1] (int64), col[nnz] (int32), hop_eV[nnz]; the diagonal is
+ * given separately in onsite_eV (diagonal entries inside the CSR arrays are rejected).
+ * kmax becomes the longest row.  Converted to the k-major list on the device. */
+int kg_create_hamiltonian_csr(kg_hamiltonian **out, int64_t n, const int64_t *rowptr,
+                              const int32_t *col, const double *hop_eV, const double *onsite_eV,
+                              const double *x_nm, double period_x_nm, double e0_eV,
+                              double scale_eV, void *stream);
+
+/* Frees the device matrix and workspace.  NULL is accepted. */
+int kg_destroy_hamiltonian(kg_hamiltonian *h);
+
+/* Bytes of device memory currently owned by the handle (matrix + workspace). */
+size_t kg_workspace_bytes(const kg_hamiltonian *h);
+
+/* Number of sites n and row width kmax of a handle (0 on NULL). */
+int64_t kg_num_sites(const kg_hamiltonian *h);
+
+/*
+ * kg_moments — Chebyshev moments C_m = <phi_L| T_m(H~) |phi_R>, m = 0..M-1, per vector
+ * (Alg. 5, eq 46).  <a|b> = sum_i conj(a_i) b_i.
+ *   phiL, phiR  [n][R]; may be the same pointer
+ *   mu          [R][M] complex128 (vector r at mu[r*M + m]), M >= 2
+ * One fused kernel per Chebyshev step (recursion eq 38 + inner product) and a final
+ * fixed-order reduction: results are bitwise reproducible run to run.
+ */
+int kg_moments(kg_hamiltonian *h, const kg_c128 *phiL, const kg_c128 *phiR, int R, int M,
+               kg_c128 *mu, void *stream);
+
+/* kg_dos_moments — C_m^DOS = <phi| T_m(H~) |phi> (eq 32; Alg. 1 l.7): kg_moments with
+ * phi_L = phi_R = phi.  For a unit-norm phi, mu_0 = 1. */
+int kg_dos_moments(kg_hamiltonian *h, const kg_c128 *phi, int R, int M, kg_c128 *mu,
+                   void *stream);
+
+/*
+ * kg_evolve — out = U(dt) in for dt_fs > 0, out = U(-|dt|) in = U^dagger(|dt|) in for dt_fs < 0
+ * (Alg. 6, eq 36), Bessel argument x = s |dt|/hbar, global phase
+ * exp(-i E0 dt/hbar).  The series keeps N_p = 1 + max{m : |J_m(x)| >= bessel_eps} terms
+ * (bessel_eps <= 0 selects 1e-15).  in, out: [n][R], out must not alias in.
+ * dt_fs = 0 is KG_EINVAL.
+ */
+int kg_evolve(kg_hamiltonian *h, const kg_c128 *in, kg_c128 *out, int R, double dt_fs,
+              double bessel_eps, void *stream);
+
+/* kg_apply_velocity — out = V in, V = (i/hbar)[H, X] with the unscaled H (eq 15):
+ * out[i] = (i/hbar) sum_k (X_{NL_ik} - X_i) H_{i,NL_ik} in[NL_ik], nm/fs. */
+int kg_apply_velocity(kg_hamiltonian *h, const kg_c128 *in, kg_c128 *out, int R, void *stream);
+
+/*
+ * kg_evolve_x — one step of eq 44, in place on caller-owned device or host arrays:
+ *   psix <- U(dt) psix + [X, U(dt)] psi,      psi <- U(dt) psi          (dt_fs > 0)
+ * with [X, U(dt)] from eq 37 and the recursions eqs 39-41 (Alg. 7).
+ * psix = 0 gives psix <- [X, U(dt)] psi.  psi, psix: [n][R].
+ */
+int kg_evolve_x(kg_hamiltonian *h, kg_c128 *psi, kg_c128 *psix, int R, double dt_fs,
+                double bessel_eps, void *stream);
+
+/*
+ * kg_vac — velocity auto-correlation moments (Alg. 2; eqs 33, 42-43):
+ *   C_m^VAC(t_k) = <phi| U(t_k) V T_m(H~) U^dagger(t_k) V |phi>,   t_k = k dt, k = 0..n_steps
+ * computed as <V psi_k| T_m(H~) |chi_k> with psi_0 = phi, chi_0 = V phi and
+ * psi_{k+1} = U(-dt) psi_k, chi_{k+1} = U(-dt) chi_k.
+ *   phi [n][R] unit-norm random vectors;  mu [R][n_steps+1][M]  (r, k, m) at
+ *   mu[(r*(n_steps+1) + k)*M + m].  dt_fs > 0, n_steps >= 0, M >= 2.
+ */
+int kg_vac(kg_hamiltonian *h, const kg_c128 *phi, int R, int M, int n_steps, double dt_fs,
+           double bessel_eps, kg_c128 *mu, void *stream);
+
+/*
+ * kg_msd — mean-square-displacement moments (Alg. 3; eqs 34, 44):
+ *   C_m^MSD(t_k) = <phi| [X,U(t_k)]^dagger T_m(H~) [X,U(t_k)] |phi>
+ * with psix_k = [X, U(t_k)] phi advanced by eq 44; row k = 0 is exactly 0.
+ * Same argument and output layout as kg_vac.
+ */
+int kg_msd(kg_hamiltonian *h, const kg_c128 *phi, int R, int M, int n_steps, double dt_fs,
+           double bessel_eps, kg_c128 *mu, void *stream);
+
+/*
+ * kg_bessel_terms — host helper exposing the series coefficients the library uses (eq 36
+ * P:200): writes N_p to *np_out and, if j != NULL, J_m(x) for m < min(N_p, cap) to
+ * the HOST array j.  Pure host arithmetic (no GPU needed).
+ */
+int kg_bessel_terms(double x, double bessel_eps, int *np_out, double *j, int cap);
+
+/* Tuning / introspection (not part of the paper's problem statement). */
+enum {
+    KG_OPT_USE_GRAPHS = 1,   /* 1 (default): replay the moment loop as a CUDA graph */
+    KG_OPT_BLOCKS_PER_SM = 2, /* persistent grid = SMs * this (default chosen per kernel) */
+    KG_OPT_THREADS = 3       /* threads per block (default 256) */
+};
+int kg_set_option(kg_hamiltonian *h, int option, int64_t value);
+
+/* Number of kernel launches (graph nodes included) the handle has enqueued since creation. */
+int64_t kg_launch_count(const kg_hamiltonian *h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KG_H */

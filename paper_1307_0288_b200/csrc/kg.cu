@@ -1,0 +1,770 @@
+// kg.cu — host side of libkg: the C ABI of include/kg.h, workspace, driver loops (a7).
+// All arithmetic on vectors runs in the kernels of kg_kernels.cuh; this file only computes the
+// O(N_p) series coefficients (Bessel functions, eq 36) on the host and enqueues kernels.
+#include "kg.h"
+#include "kg_kernels.cuh"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#define KG_HBAR 0.6582119569 /* eV fs */
+
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                        \
+    do {                                                                                      \
+        cudaError_t e_ = (expr);                                                              \
+        if (e_ != cudaSuccess)                                                                \
+            return fail(e_ == cudaErrorMemoryAllocation ? KG_ENOMEM : KG_ECUDA, "%s: %s",     \
+                        #expr, cudaGetErrorString(e_));                                       \
+    } while (0)
+
+extern "C" const char *kg_last_error(void) { return g_err; }
+
+// --------------------------------------------------------------------------------------
+// handle
+// --------------------------------------------------------------------------------------
+enum {
+    WS_TA = 0, WS_TB, WS_DA, WS_DB,        // Chebyshev vectors of the a- and d-chains
+    WS_S0, WS_S1, WS_X0, WS_X1,            // persistent time-stepping states (D6)
+    WS_PHIL,                               // V psi_k (VAC left vector)
+    WS_PART,                               // per-block moment partials [M][B][R]
+    WS_IN0, WS_IN1, WS_OUT0, WS_OUT1,      // staging for host-pointer arguments
+    WS_MU,                                 // device moments when the caller's mu is host memory
+    WS_COUNT
+};
+
+struct GraphEntry {
+    const void *phiL, *phiR;
+    int ldL, ldR, R, M, grid, threads;
+    cudaGraphExec_t exec;
+};
+
+struct kg_hamiltonian {
+    int64_t n, ns;
+    int kmax;
+    double s, e0, period;
+    bool has_onsite;
+    int32_t *nl;
+    double *hop, *xhop, *onsite;
+    void *ws[WS_COUNT];
+    size_t ws_bytes[WS_COUNT];
+    size_t matrix_bytes;
+    int device, num_sms;
+    int threads, blocks_per_sm, use_graphs;
+    int64_t launches;
+    std::vector<GraphEntry> graphs;
+};
+
+static int ws_get(kg_hamiltonian *h, int slot, size_t bytes, void **out)
+{
+    if (h->ws_bytes[slot] < bytes) {
+        if (h->ws[slot]) {
+            // a cached graph may reference the old buffer
+            for (auto &g : h->graphs) cudaGraphExecDestroy(g.exec);
+            h->graphs.clear();
+            CUDA_TRY(cudaDeviceSynchronize());
+            CUDA_TRY(cudaFree(h->ws[slot]));
+            h->ws[slot] = nullptr;
+            h->ws_bytes[slot] = 0;
+        }
+        CUDA_TRY(cudaMalloc(&h->ws[slot], bytes));
+        h->ws_bytes[slot] = bytes;
+    }
+    *out = h->ws[slot];
+    return KG_OK;
+}
+
+static bool is_device_ptr(const void *p)
+{
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+// device view of an input array: the pointer itself, or a staged copy of host memory
+static int stage_in(kg_hamiltonian *h, int slot, const void *p, size_t bytes, cudaStream_t st,
+                    const void **dev)
+{
+    if (is_device_ptr(p)) { *dev = p; return KG_OK; }
+    void *d;
+    int rc = ws_get(h, slot, bytes, &d);
+    if (rc) return rc;
+    CUDA_TRY(cudaMemcpyAsync(d, p, bytes, cudaMemcpyHostToDevice, st));
+    *dev = d;
+    return KG_OK;
+}
+
+static int grid_for(const kg_hamiltonian *h, int64_t elems)
+{
+    int64_t want = (elems + h->threads - 1) / h->threads;
+    int64_t cap = (int64_t)h->num_sms * h->blocks_per_sm;
+    if (want < 1) want = 1;
+    return (int)(want < cap ? want : cap);
+}
+
+// --------------------------------------------------------------------------------------
+// kernel dispatch
+// --------------------------------------------------------------------------------------
+template <int R, int MODE, bool FIRST>
+static cudaError_t launch_rmf(const kg_hamiltonian *h, const StepArgs &a, int grid, cudaStream_t st)
+{
+    const int th = h->threads;
+    if (h->kmax == 3) {
+        if (h->has_onsite) kg_step_kernel<R, MODE, FIRST, true, 3><<<grid, th, 0, st>>>(a);
+        else kg_step_kernel<R, MODE, FIRST, false, 3><<<grid, th, 0, st>>>(a);
+    } else {
+        if (h->has_onsite) kg_step_kernel<R, MODE, FIRST, true, 0><<<grid, th, 0, st>>>(a);
+        else kg_step_kernel<R, MODE, FIRST, false, 0><<<grid, th, 0, st>>>(a);
+    }
+    return cudaGetLastError();
+}
+
+template <int MODE, bool FIRST>
+static cudaError_t launch_mf(const kg_hamiltonian *h, int R, const StepArgs &a, int grid, cudaStream_t st)
+{
+    switch (R) {
+    case 1: return launch_rmf<1, MODE, FIRST>(h, a, grid, st);
+    case 2: return launch_rmf<2, MODE, FIRST>(h, a, grid, st);
+    case 4: return launch_rmf<4, MODE, FIRST>(h, a, grid, st);
+    case 8: return launch_rmf<8, MODE, FIRST>(h, a, grid, st);
+    case 16: return launch_rmf<16, MODE, FIRST>(h, a, grid, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+static cudaError_t launch_step(kg_hamiltonian *h, int mode, bool first, int R, const StepArgs &a,
+                               int grid, cudaStream_t st)
+{
+    h->launches++;
+    switch (mode) {
+    case MODE_MOM: return first ? launch_mf<MODE_MOM, true>(h, R, a, grid, st) : launch_mf<MODE_MOM, false>(h, R, a, grid, st);
+    case MODE_EVO: return first ? launch_mf<MODE_EVO, true>(h, R, a, grid, st) : launch_mf<MODE_EVO, false>(h, R, a, grid, st);
+    case MODE_PAIR: return first ? launch_mf<MODE_PAIR, true>(h, R, a, grid, st) : launch_mf<MODE_PAIR, false>(h, R, a, grid, st);
+    case MODE_VEL: return launch_mf<MODE_VEL, true>(h, R, a, grid, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+static StepArgs base_args(const kg_hamiltonian *h)
+{
+    StepArgs a;
+    memset(&a, 0, sizeof(a));
+    a.nl = h->nl; a.hop = h->hop; a.xhop = h->xhop; a.onsite = h->onsite;
+    a.n = h->n; a.ns = h->ns; a.kmax = h->kmax;
+    a.alpha = 2.0;
+    return a;
+}
+
+static bool r_ok(int R, bool allow16) { return R == 1 || R == 2 || R == 4 || R == 8 || (allow16 && R == 16); }
+
+// --------------------------------------------------------------------------------------
+// Bessel coefficients (R4): Miller backward recurrence in long double, normalised by
+// J_0 + 2 sum_k J_2k = 1.  N_p = 1 + max{m : |J_m(x)| >= eps}, scanned from above.
+// --------------------------------------------------------------------------------------
+static void bessel_table(double x, double eps, std::vector<double> &j)
+{
+    const double ax = std::fabs(x);
+    if (eps <= 0.0) eps = 1e-15;
+    if (ax == 0.0) { j.assign(1, 1.0); return; }
+    // start high enough that J_start/J_max is far below double rounding
+    int mtop = (int)std::ceil(ax) + 64 + (int)std::ceil(40.0 * std::cbrt(ax));
+    mtop += mtop & 1;
+    std::vector<long double> v((size_t)mtop + 2, 0.0L);
+    long double jp1 = 0.0L, jm = 1e-300L;
+    v[mtop] = jm;
+    for (int m = mtop; m >= 1; --m) {
+        const long double jm1 = (2.0L * m / (long double)ax) * jm - jp1;
+        jp1 = jm; jm = jm1;
+        v[m - 1] = jm;
+        if (fabsl(jm) > 1e300L) {                     // rescale to stay in range
+            for (int q = m - 1; q <= mtop; ++q) v[q] *= 1e-300L;
+            jm *= 1e-300L; jp1 *= 1e-300L;
+        }
+    }
+    long double norm = v[0];
+    for (int m = 2; m <= mtop; m += 2) norm += 2.0L * v[m];
+    int np = 1;
+    for (int m = mtop; m >= 0; --m)
+        if (fabsl(v[m] / norm) >= (long double)eps) { np = m + 1; break; }
+    j.resize(np);
+    for (int m = 0; m < np; ++m) {
+        double val = (double)(v[m] / norm);
+        if (x < 0.0 && (m & 1)) val = -val;           // J_m(-x) = (-1)^m J_m(x)
+        j[m] = val;
+    }
+}
+
+extern "C" int kg_bessel_terms(double x, double bessel_eps, int *np_out, double *j, int cap)
+{
+    if (!np_out || !std::isfinite(x)) return fail(KG_EINVAL, "kg_bessel_terms: bad argument");
+    std::vector<double> t;
+    bessel_table(x, bessel_eps, t);
+    *np_out = (int)t.size();
+    if (j) for (int m = 0; m < (int)t.size() && m < cap; ++m) j[m] = t[m];
+    return KG_OK;
+}
+
+// c_m = (2 - delta_m0) (-+ i)^m J_m(x) * exp(-i E0 dt/hbar), upper sign for dt > 0 (eq 36)
+static void series_coefficients(const kg_hamiltonian *h, double dt_fs, double eps, std::vector<c128> &c)
+{
+    const double xarg = h->s * std::fabs(dt_fs) / KG_HBAR;
+    std::vector<double> j;
+    bessel_table(xarg, eps, j);
+    const double ph = -h->e0 * dt_fs / KG_HBAR;
+    const double pr = std::cos(ph), pi = std::sin(ph);
+    c.resize(j.size());
+    for (size_t m = 0; m < j.size(); ++m) {
+        const double mag = (m == 0 ? 1.0 : 2.0) * j[m];
+        double re = 0.0, im = 0.0;                    // (-+ i)^m
+        switch (m & 3) {
+        case 0: re = 1.0; break;
+        case 1: im = dt_fs > 0 ? -1.0 : 1.0; break;
+        case 2: re = -1.0; break;
+        case 3: im = dt_fs > 0 ? 1.0 : -1.0; break;
+        }
+        re *= mag; im *= mag;
+        if (h->e0 != 0.0) c[m] = make_double2(re * pr - im * pi, re * pi + im * pr);
+        else c[m] = make_double2(re, im);
+    }
+}
+
+// --------------------------------------------------------------------------------------
+// create / destroy
+// --------------------------------------------------------------------------------------
+static int create_from_device_list(kg_hamiltonian **out, int64_t n, int kmax, const int32_t *d_nn,
+                                   const int32_t *d_nl, const double *d_hop, const double *d_ons,
+                                   const double *d_x, double period, double e0, double s,
+                                   cudaStream_t st)
+{
+    kg_hamiltonian *h = new (std::nothrow) kg_hamiltonian();
+    if (!h) return fail(KG_ENOMEM, "host allocation failed");
+    h->n = n; h->ns = (n + 31) / 32 * 32; h->kmax = kmax;
+    h->s = s; h->e0 = e0; h->period = period;
+    h->nl = nullptr; h->hop = h->xhop = h->onsite = nullptr;
+    memset(h->ws, 0, sizeof(h->ws));
+    memset(h->ws_bytes, 0, sizeof(h->ws_bytes));
+    h->launches = 0;
+    h->threads = 256; h->blocks_per_sm = 8; h->use_graphs = -1;
+    unsigned int *d_flags = nullptr;
+    int rc = KG_OK;
+    auto cleanup = [&](int code) { if (d_flags) cudaFree(d_flags); kg_destroy_hamiltonian(h); return code; };
+    cudaError_t e;
+    if ((e = cudaGetDevice(&h->device)) != cudaSuccess ||
+        (e = cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, h->device)) != cudaSuccess)
+        return cleanup(fail(KG_ECUDA, "device query: %s", cudaGetErrorString(e)));
+    const size_t slab = (size_t)h->ns * kmax;
+    h->matrix_bytes = slab * (4 + 8 + 8) + (size_t)h->ns * 8;
+    if ((e = cudaMalloc(&h->nl, slab * 4)) != cudaSuccess || (e = cudaMalloc(&h->hop, slab * 8)) != cudaSuccess ||
+        (e = cudaMalloc(&h->xhop, slab * 8)) != cudaSuccess || (e = cudaMalloc(&h->onsite, (size_t)h->ns * 8)) != cudaSuccess ||
+        (e = cudaMalloc(&d_flags, 16)) != cudaSuccess)
+        return cleanup(fail(KG_ENOMEM, "matrix allocation: %s", cudaGetErrorString(e)));
+    if ((e = cudaMemsetAsync(d_flags, 0, 16, st)) != cudaSuccess)
+        return cleanup(fail(KG_ECUDA, "memset: %s", cudaGetErrorString(e)));
+    const int grid = (int)std::min<int64_t>((h->ns + 255) / 256, (int64_t)h->num_sms * 8);
+    kg_build_matrix<<<grid, 256, 0, st>>>(n, h->ns, kmax, d_nn, d_nl, d_hop, d_ons, d_x, period, e0, s,
+                                          h->nl, h->hop, h->xhop, h->onsite, d_flags,
+                                          (unsigned long long *)(d_flags + 2));
+    h->launches++;
+    unsigned int host_flags[4];
+    if ((e = cudaGetLastError()) != cudaSuccess ||
+        (e = cudaMemcpyAsync(host_flags, d_flags, 16, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+        (e = cudaStreamSynchronize(st)) != cudaSuccess)
+        return cleanup(fail(KG_ECUDA, "kg_build_matrix: %s", cudaGetErrorString(e)));
+    double gersh;
+    memcpy(&gersh, host_flags + 2, 8);
+    if (host_flags[0] & 2u) rc = fail(KG_EINVAL, "nn[i] outside [0, kmax]");
+    else if (host_flags[0] & 1u) rc = fail(KG_EINVAL, "neighbour index outside [0, n)");
+    else if (host_flags[0] & 4u) rc = fail(KG_EINVAL, "non-finite hopping, on-site energy or coordinate");
+    else if (host_flags[0] & 8u) rc = fail(KG_EINVAL, "H is not symmetric (H_mi != H_im, missing reverse bond, or a diagonal entry in the list)");
+    else if (gersh > s * (1.0 + 1e-12))
+        rc = fail(KG_ESPECTRUM, "Gershgorin bound %.6g eV of (H - E0) exceeds scale %.6g eV", gersh, s);
+    if (rc) return cleanup(rc);
+    h->has_onsite = d_ons != nullptr || e0 != 0.0;
+    cudaFree(d_flags);
+    *out = h;
+    return KG_OK;
+}
+
+static int check_create_args(kg_hamiltonian **out, int64_t n, int64_t kmax, const void *a, const void *b,
+                             const void *c, const void *x, double period, double e0, double s)
+{
+    if (!out) return fail(KG_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!a || !b || !c || !x) return fail(KG_EINVAL, "NULL array argument");
+    if (n <= 0 || n >= (int64_t)1 << 31) return fail(KG_EINVAL, "n must be in [1, 2^31)");
+    if (kmax <= 0) return fail(KG_EINVAL, "kmax must be positive");
+    if (kmax > 32) return fail(KG_EUNSUPPORTED, "kmax > 32 not supported");
+    if (!(s > 0.0) || !std::isfinite(s) || !std::isfinite(e0) || !std::isfinite(period))
+        return fail(KG_EINVAL, "scale must be positive and finite; e0 and period finite");
+    return KG_OK;
+}
+
+// temporary device copies of host inputs for create
+struct TmpDev {
+    std::vector<void *> ptrs;
+    ~TmpDev() { for (void *p : ptrs) cudaFree(p); }
+    int get(const void *src, size_t bytes, cudaStream_t st, const void **dev)
+    {
+        if (!src) { *dev = nullptr; return KG_OK; }
+        if (is_device_ptr(src)) { *dev = src; return KG_OK; }
+        void *d = nullptr;
+        CUDA_TRY(cudaMalloc(&d, bytes));
+        ptrs.push_back(d);
+        CUDA_TRY(cudaMemcpyAsync(d, src, bytes, cudaMemcpyHostToDevice, st));
+        *dev = d;
+        return KG_OK;
+    }
+};
+
+extern "C" int kg_create_hamiltonian(kg_hamiltonian **out, int64_t n, int32_t kmax, const int32_t *nn,
+                                     const int32_t *nl, const double *hop_eV, const double *onsite_eV,
+                                     const double *x_nm, double period_x_nm, double e0_eV,
+                                     double scale_eV, void *stream)
+{
+    int rc = check_create_args(out, n, kmax, nn, nl, hop_eV, x_nm, period_x_nm, e0_eV, scale_eV);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    TmpDev tmp;
+    const void *d_nn, *d_nl, *d_hop, *d_ons, *d_x;
+    if ((rc = tmp.get(nn, (size_t)n * 4, st, &d_nn)) || (rc = tmp.get(nl, (size_t)n * kmax * 4, st, &d_nl)) ||
+        (rc = tmp.get(hop_eV, (size_t)n * kmax * 8, st, &d_hop)) || (rc = tmp.get(onsite_eV, (size_t)n * 8, st, &d_ons)) ||
+        (rc = tmp.get(x_nm, (size_t)n * 8, st, &d_x)))
+        return rc;
+    return create_from_device_list(out, n, kmax, (const int32_t *)d_nn, (const int32_t *)d_nl,
+                                   (const double *)d_hop, (const double *)d_ons, (const double *)d_x,
+                                   period_x_nm, e0_eV, scale_eV, st);
+}
+
+extern "C" int kg_create_hamiltonian_csr(kg_hamiltonian **out, int64_t n, const int64_t *rowptr,
+                                         const int32_t *col, const double *hop_eV,
+                                         const double *onsite_eV, const double *x_nm,
+                                         double period_x_nm, double e0_eV, double scale_eV, void *stream)
+{
+    int rc = check_create_args(out, n, 1, rowptr, col, hop_eV, x_nm, period_x_nm, e0_eV, scale_eV);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    TmpDev tmp;
+    const void *d_rp, *d_col, *d_val, *d_ons, *d_x;
+    if ((rc = tmp.get(rowptr, (size_t)(n + 1) * 8, st, &d_rp))) return rc;
+    int64_t nnz = 0;
+    CUDA_TRY(cudaMemcpyAsync(&nnz, (const int64_t *)d_rp + n, 8, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (nnz < 0 || nnz > n * 32) return fail(KG_EINVAL, "rowptr[n] = %lld is not a valid nnz", (long long)nnz);
+    const size_t nz = (size_t)(nnz > 0 ? nnz : 1);
+    if ((rc = tmp.get(col, nz * 4, st, &d_col)) || (rc = tmp.get(hop_eV, nz * 8, st, &d_val)) ||
+        (rc = tmp.get(onsite_eV, (size_t)n * 8, st, &d_ons)) || (rc = tmp.get(x_nm, (size_t)n * 8, st, &d_x)))
+        return rc;
+    int *d_max = nullptr;
+    CUDA_TRY(cudaMalloc(&d_max, 8));
+    tmp.ptrs.push_back(d_max);
+    CUDA_TRY(cudaMemsetAsync(d_max, 0, 8, st));
+    const int grid = (int)std::min<int64_t>((n + 255) / 256, 1184);
+    kg_csr_max_row<<<grid, 256, 0, st>>>(n, (const int64_t *)d_rp, d_max, (unsigned int *)(d_max + 1));
+    int hostv[2];
+    CUDA_TRY(cudaMemcpyAsync(hostv, d_max, 8, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (hostv[1]) return fail(KG_EINVAL, "CSR row length outside [0, 32]");
+    const int kmax = hostv[0] > 0 ? hostv[0] : 1;
+    int32_t *d_nn = nullptr, *d_nl = nullptr;
+    double *d_hop = nullptr;
+    CUDA_TRY(cudaMalloc(&d_nn, (size_t)n * 4)); tmp.ptrs.push_back(d_nn);
+    CUDA_TRY(cudaMalloc(&d_nl, (size_t)n * kmax * 4)); tmp.ptrs.push_back(d_nl);
+    CUDA_TRY(cudaMalloc(&d_hop, (size_t)n * kmax * 8)); tmp.ptrs.push_back(d_hop);
+    kg_csr_to_ell<<<grid, 256, 0, st>>>(n, (const int64_t *)d_rp, (const int32_t *)d_col,
+                                        (const double *)d_val, kmax, d_nn, d_nl, d_hop);
+    CUDA_TRY(cudaGetLastError());
+    return create_from_device_list(out, n, kmax, d_nn, d_nl, d_hop, (const double *)d_ons,
+                                   (const double *)d_x, period_x_nm, e0_eV, scale_eV, st);
+}
+
+extern "C" int kg_destroy_hamiltonian(kg_hamiltonian *h)
+{
+    if (!h) return KG_OK;
+    for (auto &g : h->graphs) cudaGraphExecDestroy(g.exec);
+    cudaFree(h->nl); cudaFree(h->hop); cudaFree(h->xhop); cudaFree(h->onsite);
+    for (int i = 0; i < WS_COUNT; ++i) cudaFree(h->ws[i]);
+    delete h;
+    return KG_OK;
+}
+
+extern "C" size_t kg_workspace_bytes(const kg_hamiltonian *h)
+{
+    if (!h) return 0;
+    size_t t = h->matrix_bytes;
+    for (int i = 0; i < WS_COUNT; ++i) t += h->ws_bytes[i];
+    return t;
+}
+
+extern "C" int64_t kg_num_sites(const kg_hamiltonian *h) { return h ? h->n : 0; }
+extern "C" int64_t kg_launch_count(const kg_hamiltonian *h) { return h ? h->launches : 0; }
+
+extern "C" int kg_set_option(kg_hamiltonian *h, int option, int64_t value)
+{
+    if (!h) return fail(KG_EINVAL, "NULL handle");
+    switch (option) {
+    case KG_OPT_USE_GRAPHS: h->use_graphs = (int)value; break;
+    case KG_OPT_BLOCKS_PER_SM:
+        if (value < 1 || value > 32) return fail(KG_EINVAL, "blocks per SM must be in [1, 32]");
+        h->blocks_per_sm = (int)value; break;
+    case KG_OPT_THREADS:
+        if (value != 64 && value != 128 && value != 256) return fail(KG_EINVAL, "threads must be 64, 128 or 256");
+        h->threads = (int)value; break;
+    default: return fail(KG_EINVAL, "unknown option %d", option);
+    }
+    for (auto &g : h->graphs) cudaGraphExecDestroy(g.exec);
+    h->graphs.clear();
+    return KG_OK;
+}
+
+// --------------------------------------------------------------------------------------
+// device-level drivers (all pointers are device pointers here)
+// --------------------------------------------------------------------------------------
+
+// enqueue the M-1 fused recursion+dot kernels of Alg. 5 (a2+a3); partials [M][grid][R]
+static int enqueue_moment_steps(kg_hamiltonian *h, const c128 *phiL, int ldL, const c128 *phiR, int ldR,
+                                int R, int M, c128 *ta, c128 *tb, c128 *part, int grid, cudaStream_t st)
+{
+    const size_t prow = (size_t)grid * R;
+    StepArgs a = base_args(h);
+    a.phiL = phiL; a.ld_L = ldL;
+    // m = 1: T_1 = H~ T_0, partial rows 0 and 1
+    a.alpha = 1.0;
+    a.cur = phiR; a.ld_cur = ldR; a.next = ta;
+    a.partial0 = part; a.partial = part + prow;
+    CUDA_TRY(launch_step(h, MODE_MOM, true, R, a, grid, st));
+    a.alpha = 2.0; a.partial0 = nullptr;
+    for (int m = 2; m < M; ++m) {
+        a.partial = part + (size_t)m * prow;
+        if (m == 2) { a.cur = ta; a.ld_cur = R; a.prev = phiR; a.ld_prev = ldR; a.next = tb; }
+        else if (m & 1) { a.cur = tb; a.ld_cur = R; a.prev = ta; a.ld_prev = R; a.next = ta; }
+        else { a.cur = ta; a.ld_cur = R; a.prev = tb; a.ld_prev = R; a.next = tb; }
+        CUDA_TRY(launch_step(h, MODE_MOM, false, R, a, grid, st));
+    }
+    return KG_OK;
+}
+
+static bool want_graph(const kg_hamiltonian *h, int64_t elems, cudaStream_t st)
+{
+    // the legacy default stream cannot be captured
+    if (st == nullptr || st == cudaStreamLegacy || h->use_graphs == 0) return false;
+    if (h->use_graphs > 0) return true;
+    return elems <= (int64_t)1 << 21;      // auto: launch-bound sizes only
+}
+
+// mu[r*mu_rstride + m] = <phiL_r | T_m(H~) | phiR_r>, m < M
+static int moments_device(kg_hamiltonian *h, const c128 *phiL, int ldL, const c128 *phiR, int ldR, int R,
+                          int M, c128 *mu, int64_t mu_rstride, cudaStream_t st)
+{
+    const int64_t elems = h->n * R;
+    const int grid = grid_for(h, elems);
+    void *ta, *tb, *part;
+    int rc;
+    if ((rc = ws_get(h, WS_TA, (size_t)elems * 16, &ta)) || (rc = ws_get(h, WS_TB, (size_t)elems * 16, &tb)) ||
+        (rc = ws_get(h, WS_PART, (size_t)M * grid * R * 16, &part)))
+        return rc;
+    if (want_graph(h, elems, st)) {
+        cudaGraphExec_t exec = nullptr;
+        for (auto &g : h->graphs)
+            if (g.phiL == phiL && g.phiR == phiR && g.ldL == ldL && g.ldR == ldR && g.R == R && g.M == M &&
+                g.grid == grid && g.threads == h->threads)
+                exec = g.exec;
+        if (!exec) {
+            cudaGraph_t graph;
+            CUDA_TRY(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+            const int64_t before = h->launches;
+            rc = enqueue_moment_steps(h, phiL, ldL, phiR, ldR, R, M, (c128 *)ta, (c128 *)tb, (c128 *)part, grid, st);
+            h->launches = before;
+            cudaError_t e = cudaStreamEndCapture(st, &graph);
+            if (rc) { if (e == cudaSuccess) cudaGraphDestroy(graph); return rc; }
+            if (e != cudaSuccess) return fail(KG_ECUDA, "graph capture: %s", cudaGetErrorString(e));
+            e = cudaGraphInstantiate(&exec, graph, 0);
+            cudaGraphDestroy(graph);
+            if (e != cudaSuccess) return fail(KG_ECUDA, "graph instantiate: %s", cudaGetErrorString(e));
+            if (h->graphs.size() >= 8) { cudaGraphExecDestroy(h->graphs.front().exec); h->graphs.erase(h->graphs.begin()); }
+            h->graphs.push_back(GraphEntry{phiL, phiR, ldL, ldR, R, M, grid, h->threads, exec});
+        }
+        CUDA_TRY(cudaGraphLaunch(exec, st));
+        h->launches += M - 1;
+    } else {
+        if ((rc = enqueue_moment_steps(h, phiL, ldL, phiR, ldR, R, M, (c128 *)ta, (c128 *)tb, (c128 *)part, grid, st)))
+            return rc;
+    }
+    const int warps = M * R;
+    kg_reduce_partials<<<(warps * 32 + 255) / 256, 256, 0, st>>>((const c128 *)part, M, grid, R, mu, mu_rstride);
+    h->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return KG_OK;
+}
+
+// out = U(dt) in  (Alg. 6): in [n] with row stride ld_in, out [n][R]
+static int evolve_device(kg_hamiltonian *h, const c128 *in, int ld_in, c128 *out, int R, double dt_fs,
+                         double eps, cudaStream_t st)
+{
+    const int64_t elems = h->n * R;
+    const int grid = grid_for(h, elems);
+    void *ta, *tb;
+    int rc;
+    if ((rc = ws_get(h, WS_TA, (size_t)elems * 16, &ta)) || (rc = ws_get(h, WS_TB, (size_t)elems * 16, &tb))) return rc;
+    std::vector<c128> c;
+    series_coefficients(h, dt_fs, eps, c);
+    const int np = (int)c.size();
+    StepArgs a = base_args(h);
+    a.out = out;
+    a.alpha = 1.0;
+    a.cur = in; a.ld_cur = ld_in; a.next = (c128 *)ta;
+    a.c0 = c[0]; a.c1 = np > 1 ? c[1] : make_double2(0.0, 0.0);
+    CUDA_TRY(launch_step(h, MODE_EVO, true, R, a, grid, st));
+    a.alpha = 2.0;
+    for (int m = 2; m < np; ++m) {
+        a.c1 = c[m];
+        if (m == 2) { a.cur = (c128 *)ta; a.ld_cur = R; a.prev = in; a.ld_prev = ld_in; a.next = (c128 *)tb; }
+        else if (m & 1) { a.cur = (c128 *)tb; a.prev = (c128 *)ta; a.ld_prev = R; a.next = (c128 *)ta; }
+        else { a.cur = (c128 *)ta; a.prev = (c128 *)tb; a.ld_prev = R; a.next = (c128 *)tb; }
+        CUDA_TRY(launch_step(h, MODE_EVO, false, R, a, grid, st));
+    }
+    return KG_OK;
+}
+
+// (psi_out, psix_out) = (U psi, U psix + [X,U] psi)  (eq 44 via the (a,d) pair recursion)
+static int pair_device(kg_hamiltonian *h, const c128 *psi, const c128 *psix, c128 *psi_out, c128 *psix_out,
+                       int R, double dt_fs, double eps, cudaStream_t st)
+{
+    const int64_t elems = h->n * R;
+    const int grid = grid_for(h, elems);
+    void *ta, *tb, *da, *db;
+    int rc;
+    if ((rc = ws_get(h, WS_TA, (size_t)elems * 16, &ta)) || (rc = ws_get(h, WS_TB, (size_t)elems * 16, &tb)) ||
+        (rc = ws_get(h, WS_DA, (size_t)elems * 16, &da)) || (rc = ws_get(h, WS_DB, (size_t)elems * 16, &db)))
+        return rc;
+    std::vector<c128> c;
+    series_coefficients(h, dt_fs, eps, c);
+    const int np = (int)c.size();
+    StepArgs a = base_args(h);
+    a.out = psi_out; a.outd = psix_out;
+    a.alpha = 1.0;
+    a.cur = psi; a.ld_cur = R; a.next = (c128 *)ta;
+    a.dcur = psix; a.ld_dcur = R; a.dnext = (c128 *)da;
+    a.c0 = c[0]; a.c1 = np > 1 ? c[1] : make_double2(0.0, 0.0);
+    CUDA_TRY(launch_step(h, MODE_PAIR, true, R, a, grid, st));
+    a.alpha = 2.0;
+    a.ld_prev = R; a.ld_dprev = R;
+    for (int m = 2; m < np; ++m) {
+        a.c1 = c[m];
+        if (m == 2) {
+            a.cur = (c128 *)ta; a.prev = psi; a.next = (c128 *)tb;
+            a.dcur = (c128 *)da; a.dprev = psix; a.dnext = (c128 *)db;
+        } else if (m & 1) {
+            a.cur = (c128 *)tb; a.prev = (c128 *)ta; a.next = (c128 *)ta;
+            a.dcur = (c128 *)db; a.dprev = (c128 *)da; a.dnext = (c128 *)da;
+        } else {
+            a.cur = (c128 *)ta; a.prev = (c128 *)tb; a.next = (c128 *)tb;
+            a.dcur = (c128 *)da; a.dprev = (c128 *)db; a.dnext = (c128 *)db;
+        }
+        CUDA_TRY(launch_step(h, MODE_PAIR, false, R, a, grid, st));
+    }
+    return KG_OK;
+}
+
+static int velocity_device(kg_hamiltonian *h, const c128 *in, int ld_in, c128 *out, int ld_out, int R,
+                           cudaStream_t st)
+{
+    StepArgs a = base_args(h);
+    a.cur = in; a.ld_cur = ld_in; a.vout = out; a.ld_vout = ld_out;
+    a.vscale = h->s / KG_HBAR;
+    CUDA_TRY(launch_step(h, MODE_VEL, true, R, a, grid_for(h, h->n * R), st));
+    return KG_OK;
+}
+
+static int copy_cols(kg_hamiltonian *h, const c128 *src, int ld_src, c128 *dst, int ld_dst, int ncols,
+                     cudaStream_t st)
+{
+    kg_copy_cols<<<grid_for(h, h->n * ncols), h->threads, 0, st>>>(src, ld_src, dst, ld_dst, ncols, h->n);
+    h->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return KG_OK;
+}
+
+// output staging: device buffer to compute into, copied to the caller's host array afterwards
+struct OutStage { void *user; void *dev; size_t bytes; bool host; };
+static int stage_out(kg_hamiltonian *h, int slot, void *p, size_t bytes, OutStage *o)
+{
+    o->user = p; o->bytes = bytes; o->host = !is_device_ptr(p);
+    if (!o->host) { o->dev = p; return KG_OK; }
+    return ws_get(h, slot, bytes, &o->dev);
+}
+static int finish_out(const OutStage &o, cudaStream_t st)
+{
+    if (o.host) CUDA_TRY(cudaMemcpyAsync(o.user, o.dev, o.bytes, cudaMemcpyDeviceToHost, st));
+    return KG_OK;
+}
+
+// --------------------------------------------------------------------------------------
+// public calls
+// --------------------------------------------------------------------------------------
+extern "C" int kg_moments(kg_hamiltonian *h, const kg_c128 *phiL, const kg_c128 *phiR, int R, int M,
+                          kg_c128 *mu, void *stream)
+{
+    if (!h || !phiL || !phiR || !mu) return fail(KG_EINVAL, "kg_moments: NULL argument");
+    if (!r_ok(R, false)) return fail(KG_EUNSUPPORTED, "R must be 1, 2, 4 or 8");
+    if (M < 2) return fail(KG_EINVAL, "M must be >= 2");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t vbytes = (size_t)h->n * R * 16;
+    const void *dL, *dR;
+    int rc;
+    if ((rc = stage_in(h, WS_IN0, phiL, vbytes, st, &dL))) return rc;
+    if (phiR == phiL) dR = dL;
+    else if ((rc = stage_in(h, WS_IN1, phiR, vbytes, st, &dR))) return rc;
+    OutStage o;
+    if ((rc = stage_out(h, WS_MU, mu, (size_t)R * M * 16, &o))) return rc;
+    if ((rc = moments_device(h, (const c128 *)dL, R, (const c128 *)dR, R, R, M, (c128 *)o.dev, M, st))) return rc;
+    return finish_out(o, st);
+}
+
+extern "C" int kg_dos_moments(kg_hamiltonian *h, const kg_c128 *phi, int R, int M, kg_c128 *mu, void *stream)
+{
+    return kg_moments(h, phi, phi, R, M, mu, stream);
+}
+
+extern "C" int kg_evolve(kg_hamiltonian *h, const kg_c128 *in, kg_c128 *out, int R, double dt_fs,
+                         double bessel_eps, void *stream)
+{
+    if (!h || !in || !out) return fail(KG_EINVAL, "kg_evolve: NULL argument");
+    if (in == out) return fail(KG_EINVAL, "kg_evolve: out must not alias in");
+    if (!r_ok(R, true)) return fail(KG_EUNSUPPORTED, "R must be 1, 2, 4, 8 or 16");
+    if (dt_fs == 0.0 || !std::isfinite(dt_fs)) return fail(KG_EINVAL, "dt_fs must be finite and non-zero");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t vbytes = (size_t)h->n * R * 16;
+    const void *din;
+    OutStage o;
+    int rc;
+    if ((rc = stage_in(h, WS_IN0, in, vbytes, st, &din)) || (rc = stage_out(h, WS_OUT0, out, vbytes, &o))) return rc;
+    if ((rc = evolve_device(h, (const c128 *)din, R, (c128 *)o.dev, R, dt_fs, bessel_eps, st))) return rc;
+    return finish_out(o, st);
+}
+
+extern "C" int kg_apply_velocity(kg_hamiltonian *h, const kg_c128 *in, kg_c128 *out, int R, void *stream)
+{
+    if (!h || !in || !out) return fail(KG_EINVAL, "kg_apply_velocity: NULL argument");
+    if (in == out) return fail(KG_EINVAL, "kg_apply_velocity: out must not alias in");
+    if (!r_ok(R, true)) return fail(KG_EUNSUPPORTED, "R must be 1, 2, 4, 8 or 16");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t vbytes = (size_t)h->n * R * 16;
+    const void *din;
+    OutStage o;
+    int rc;
+    if ((rc = stage_in(h, WS_IN0, in, vbytes, st, &din)) || (rc = stage_out(h, WS_OUT0, out, vbytes, &o))) return rc;
+    if ((rc = velocity_device(h, (const c128 *)din, R, (c128 *)o.dev, R, R, st))) return rc;
+    return finish_out(o, st);
+}
+
+extern "C" int kg_evolve_x(kg_hamiltonian *h, kg_c128 *psi, kg_c128 *psix, int R, double dt_fs,
+                           double bessel_eps, void *stream)
+{
+    if (!h || !psi || !psix) return fail(KG_EINVAL, "kg_evolve_x: NULL argument");
+    if (psi == psix) return fail(KG_EINVAL, "kg_evolve_x: psi and psix must be distinct");
+    if (!r_ok(R, false)) return fail(KG_EUNSUPPORTED, "R must be 1, 2, 4 or 8");
+    if (!(dt_fs > 0.0) || !std::isfinite(dt_fs)) return fail(KG_EINVAL, "dt_fs must be finite and positive");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t vbytes = (size_t)h->n * R * 16;
+    const void *dpsi, *dpsix;
+    void *o0, *o1;
+    int rc;
+    if ((rc = stage_in(h, WS_IN0, psi, vbytes, st, &dpsi)) || (rc = stage_in(h, WS_IN1, psix, vbytes, st, &dpsix)) ||
+        (rc = ws_get(h, WS_OUT0, vbytes, &o0)) || (rc = ws_get(h, WS_OUT1, vbytes, &o1)))
+        return rc;
+    if ((rc = pair_device(h, (const c128 *)dpsi, (const c128 *)dpsix, (c128 *)o0, (c128 *)o1, R, dt_fs, bessel_eps, st)))
+        return rc;
+    CUDA_TRY(cudaMemcpyAsync(psi, o0, vbytes, cudaMemcpyDefault, st));
+    CUDA_TRY(cudaMemcpyAsync(psix, o1, vbytes, cudaMemcpyDefault, st));
+    return KG_OK;
+}
+
+static int check_corr_args(kg_hamiltonian *h, const void *phi, int R, int M, int n_steps, double dt_fs, void *mu)
+{
+    if (!h || !phi || !mu) return fail(KG_EINVAL, "NULL argument");
+    if (!r_ok(R, false)) return fail(KG_EUNSUPPORTED, "R must be 1, 2, 4 or 8");
+    if (M < 2) return fail(KG_EINVAL, "M must be >= 2");
+    if (n_steps < 0) return fail(KG_EINVAL, "n_steps must be >= 0");
+    if (!(dt_fs > 0.0) || !std::isfinite(dt_fs)) return fail(KG_EINVAL, "dt_fs must be finite and positive");
+    return KG_OK;
+}
+
+extern "C" int kg_vac(kg_hamiltonian *h, const kg_c128 *phi, int R, int M, int n_steps, double dt_fs,
+                      double bessel_eps, kg_c128 *mu, void *stream)
+{
+    int rc = check_corr_args(h, phi, R, M, n_steps, dt_fs, mu);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t vbytes = (size_t)h->n * R * 16;
+    const int R2 = 2 * R;
+    const void *dphi;
+    void *s0, *s1, *pl;
+    OutStage o;
+    if ((rc = stage_in(h, WS_IN0, phi, vbytes, st, &dphi)) || (rc = ws_get(h, WS_S0, 2 * vbytes, &s0)) ||
+        (rc = ws_get(h, WS_S1, 2 * vbytes, &s1)) || (rc = ws_get(h, WS_PHIL, vbytes, &pl)) ||
+        (rc = stage_out(h, WS_MU, mu, (size_t)R * (n_steps + 1) * M * 16, &o)))
+        return rc;
+    // state S = [psi | chi] as one [n][2R] batch: psi_0 = phi, chi_0 = V phi  (Alg. 2)
+    c128 *S = (c128 *)s0, *Sn = (c128 *)s1;
+    if ((rc = copy_cols(h, (const c128 *)dphi, R, S, R2, R, st)) ||
+        (rc = velocity_device(h, (const c128 *)dphi, R, S + R, R2, R, st)))
+        return rc;
+    const int64_t rstride = (int64_t)(n_steps + 1) * M;
+    for (int k = 0; k <= n_steps; ++k) {
+        // phi_L = V psi_k, phi_R = chi_k
+        if ((rc = velocity_device(h, S, R2, (c128 *)pl, R, R, st)) ||
+            (rc = moments_device(h, (const c128 *)pl, R, S + R, R2, R, M, (c128 *)o.dev + (size_t)k * M, rstride, st)))
+            return rc;
+        if (k == n_steps) break;
+        // [psi | chi] <- U(-dt) [psi | chi]   (eqs 42-43), one 2R-wide batch
+        if ((rc = evolve_device(h, S, R2, Sn, R2, -dt_fs, bessel_eps, st))) return rc;
+        c128 *t = S; S = Sn; Sn = t;
+    }
+    return finish_out(o, st);
+}
+
+extern "C" int kg_msd(kg_hamiltonian *h, const kg_c128 *phi, int R, int M, int n_steps, double dt_fs,
+                      double bessel_eps, kg_c128 *mu, void *stream)
+{
+    int rc = check_corr_args(h, phi, R, M, n_steps, dt_fs, mu);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t vbytes = (size_t)h->n * R * 16;
+    const void *dphi;
+    void *p0, *p1, *x0, *x1;
+    OutStage o;
+    if ((rc = stage_in(h, WS_IN0, phi, vbytes, st, &dphi)) || (rc = ws_get(h, WS_S0, vbytes, &p0)) ||
+        (rc = ws_get(h, WS_S1, vbytes, &p1)) || (rc = ws_get(h, WS_X0, vbytes, &x0)) ||
+        (rc = ws_get(h, WS_X1, vbytes, &x1)) ||
+        (rc = stage_out(h, WS_MU, mu, (size_t)R * (n_steps + 1) * M * 16, &o)))
+        return rc;
+    c128 *P = (c128 *)p0, *Pn = (c128 *)p1, *X = (c128 *)x0, *Xn = (c128 *)x1;
+    CUDA_TRY(cudaMemcpyAsync(P, dphi, vbytes, cudaMemcpyDeviceToDevice, st));   // psi_0 = phi
+    CUDA_TRY(cudaMemsetAsync(X, 0, vbytes, st));                                // psix_0 = 0
+    const int64_t rstride = (int64_t)(n_steps + 1) * M;
+    for (int k = 0; k <= n_steps; ++k) {
+        if ((rc = moments_device(h, X, R, X, R, R, M, (c128 *)o.dev + (size_t)k * M, rstride, st))) return rc;
+        if (k == n_steps) break;
+        if ((rc = pair_device(h, P, X, Pn, Xn, R, dt_fs, bessel_eps, st))) return rc;
+        c128 *t = P; P = Pn; Pn = t;
+        t = X; X = Xn; Xn = t;
+    }
+    return finish_out(o, st);
+}

@@ -1,0 +1,331 @@
+// kg_kernels.cuh — device kernels of libkg (sm_100a).
+//
+// One fused kernel family implements every step of the hot path:
+//
+//   MODE_MOM   T_{m+1} = alpha H~ T_m - beta T_{m-1}  (eq 38)  + per-block partial of
+//              <phi_L|T_{m+1}>  (Alg. 5 l.6-7 P:363-365; the paper's K3 and K5 in one pass)
+//   MODE_EVO   same recursion + out (+)= c_{m+1} T_{m+1}              (Alg. 6 l.5-6 P:383-385)
+//   MODE_PAIR  (a, d) pair recursion: a = T_m psi, d = T_m psix + [X,T_m] psi,
+//              d_{m+1} = alpha([X,H~] a_m + H~ d_m) - beta d_{m-1}    (eq 39, Alg. 7 l.7-8)
+//              + both series accumulations                            (eq 44)
+//   MODE_VEL   out = V in = -(i s/hbar) [X,H~] in                     (eq 15)
+//
+// Layout: vectors [n][R] complex128 (double2), one THREAD PER ELEMENT (site i, vector r),
+// e = i*R + r, so the R lanes of a site read R consecutive 16-byte values: every own-element
+// access is a fully coalesced ld.global.v2.f64, every gather reads R*16 contiguous bytes, and
+// the matrix row (index, hopping, on-site) is fetched once per site and broadcast to R lanes.
+// The matrix is the paper's k-major neighbour list with row stride `ns` (n rounded up
+// to 32 so that each k-slab is 128-byte aligned).
+//
+// Determinism: a thread's elements are fixed by (grid, block), per-thread sums run in index
+// order, the warp/block reduction is a fixed tree, and kg_reduce_partials adds the per-block
+// partials in block order: moments are bitwise reproducible.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+typedef double2 c128;
+
+enum { MODE_MOM = 0, MODE_EVO = 1, MODE_PAIR = 2, MODE_VEL = 3 };
+
+struct StepArgs {
+    // matrix (device, library-owned)
+    const int32_t *nl;    // [kmax][ns]
+    const double *hop;    // [kmax][ns]  H_ik / s
+    const double *xhop;   // [kmax][ns]  (X_i - X_m)_minimg H_ik / s   ([X,H~] weights)
+    const double *onsite; // [ns]        (H_ii - E0)/s
+    int64_t n;            // sites
+    int64_t ns;           // row stride of the k-major arrays
+    int kmax;
+    double alpha;         // 1 for the first step (T_1 = H~ T_0), 2 afterwards
+    // a-chain: element (i, r) of X at X[i*ld + r]
+    const c128 *cur;  int ld_cur;    // T_m      (gathered + own)
+    const c128 *prev; int ld_prev;   // T_{m-1}  (own element; unused when FIRST)
+    c128 *next;                      // T_{m+1}  (ld = R); may alias prev
+    // MODE_MOM
+    const c128 *phiL; int ld_L;
+    c128 *partial;                   // [grid][R] for moment m+1
+    c128 *partial0;                  // FIRST only: [grid][R] for moment 0
+    // MODE_EVO / MODE_PAIR: series accumulators (ld = R)
+    c128 *out;
+    c128 c0, c1;                     // FIRST: out = c0 cur + c1 next; else out += c1 next
+    // MODE_PAIR d-chain
+    const c128 *dcur; int ld_dcur;
+    const c128 *dprev; int ld_dprev;
+    c128 *dnext;
+    c128 *outd;
+    // MODE_VEL
+    c128 *vout; int ld_vout;
+    double vscale;                   // s / hbar
+};
+
+__device__ __forceinline__ c128 ld_nc(const c128 *p)
+{
+    return __ldg(reinterpret_cast<const double2 *>(p));
+}
+__device__ __forceinline__ c128 cmul(c128 a, c128 b)
+{
+    return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+__device__ __forceinline__ void cfma_r(c128 &acc, double h, c128 v)
+{
+    acc.x = fma(h, v.x, acc.x);
+    acc.y = fma(h, v.y, acc.y);
+}
+
+// Sum `v` over the lanes of a warp that share (lane % R), then over warps; thread tid < R of
+// the block ends up with the block total for vector r = tid.  Fixed tree => deterministic.
+template <int R>
+__device__ __forceinline__ c128 block_reduce_per_r(c128 v, c128 *smem /* [32][R] */)
+{
+#pragma unroll
+    for (int off = 16; off >= R; off >>= 1) {
+        v.x += __shfl_xor_sync(0xffffffffu, v.x, off);
+        v.y += __shfl_xor_sync(0xffffffffu, v.y, off);
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int nwarps = blockDim.x >> 5;
+    if (lane < R) smem[warp * R + lane] = v;
+    __syncthreads();
+    c128 tot = make_double2(0.0, 0.0);
+    if (threadIdx.x < R) {
+        for (int w = 0; w < nwarps; ++w) {
+            tot.x += smem[w * R + threadIdx.x].x;
+            tot.y += smem[w * R + threadIdx.x].y;
+        }
+    }
+    __syncthreads();
+    return tot;
+}
+
+// R = 16 or 32 lanes would leave nothing to shuffle for R = 32; supported R: 1, 2, 4, 8, 16.
+template <int R, int MODE, bool FIRST, bool ONS, int KMAX>
+__global__ void __launch_bounds__(256) kg_step_kernel(const StepArgs a)
+{
+    const int64_t total = a.n * R;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    const int r = threadIdx.x & (R - 1);
+    const int kmax = KMAX > 0 ? KMAX : a.kmax;
+
+    c128 sum = make_double2(0.0, 0.0), sum0 = make_double2(0.0, 0.0);
+
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += stride) {
+        const int64_t i = e / R;   // R is a power of two: a shift
+        c128 acc = make_double2(0.0, 0.0);
+        c128 dacc = make_double2(0.0, 0.0);
+        c128 self = make_double2(0.0, 0.0), dself = make_double2(0.0, 0.0);
+        if (MODE != MODE_VEL && (ONS || FIRST)) {
+            self = ld_nc(a.cur + i * a.ld_cur + r);
+            if (MODE == MODE_PAIR) dself = ld_nc(a.dcur + i * a.ld_dcur + r);
+        }
+        if (MODE != MODE_VEL && ONS) {
+            const double eps = __ldg(a.onsite + i);
+            acc.x = eps * self.x; acc.y = eps * self.y;
+            if (MODE == MODE_PAIR) { dacc.x = eps * dself.x; dacc.y = eps * dself.y; }
+        }
+#pragma unroll
+        for (int k = 0; k < kmax; ++k) {
+            const int64_t m = __ldg(a.nl + k * a.ns + i);
+            if (MODE == MODE_VEL) {
+                const double w = __ldg(a.xhop + k * a.ns + i);
+                cfma_r(acc, w, ld_nc(a.cur + m * a.ld_cur + r));
+            } else {
+                const double h = __ldg(a.hop + k * a.ns + i);
+                const c128 v = ld_nc(a.cur + m * a.ld_cur + r);
+                cfma_r(acc, h, v);
+                if (MODE == MODE_PAIR) {
+                    const double w = __ldg(a.xhop + k * a.ns + i);
+                    cfma_r(dacc, w, v);                                   // [X,H~] a_m
+                    cfma_r(dacc, h, ld_nc(a.dcur + m * a.ld_dcur + r));   // H~ d_m
+                }
+            }
+        }
+        if (MODE == MODE_VEL) {
+            // V = -(i s/hbar)[X,H~]:  -i (x + i y) = y - i x
+            a.vout[i * a.ld_vout + r] = make_double2(a.vscale * acc.y, -a.vscale * acc.x);
+            continue;
+        }
+        c128 t;
+        if (FIRST) {
+            t = acc;
+        } else {
+            const c128 p = a.prev[i * a.ld_prev + r];
+            t = make_double2(fma(a.alpha, acc.x, -p.x), fma(a.alpha, acc.y, -p.y));
+        }
+        a.next[e] = t;
+        if (MODE == MODE_MOM) {
+            const c128 L = ld_nc(a.phiL + i * a.ld_L + r);
+            sum.x = fma(L.x, t.x, fma(L.y, t.y, sum.x));      // conj(L) * t
+            sum.y = fma(L.x, t.y, fma(-L.y, t.x, sum.y));
+            if (FIRST) {
+                sum0.x = fma(L.x, self.x, fma(L.y, self.y, sum0.x));
+                sum0.y = fma(L.x, self.y, fma(-L.y, self.x, sum0.y));
+            }
+        }
+        if (MODE == MODE_EVO || MODE == MODE_PAIR) {
+            c128 o;
+            if (FIRST) o = cmul(a.c0, self); else o = a.out[e];
+            const c128 ct = cmul(a.c1, t);
+            a.out[e] = make_double2(o.x + ct.x, o.y + ct.y);
+        }
+        if (MODE == MODE_PAIR) {
+            c128 dt;
+            if (FIRST) {
+                dt = dacc;
+            } else {
+                const c128 p = a.dprev[i * a.ld_dprev + r];
+                dt = make_double2(fma(a.alpha, dacc.x, -p.x), fma(a.alpha, dacc.y, -p.y));
+            }
+            a.dnext[e] = dt;
+            c128 o;
+            if (FIRST) o = cmul(a.c0, dself); else o = a.outd[e];
+            const c128 ct = cmul(a.c1, dt);
+            a.outd[e] = make_double2(o.x + ct.x, o.y + ct.y);
+        }
+    }
+
+    if (MODE == MODE_MOM) {
+        __shared__ c128 red[32 * R];
+        c128 tot = block_reduce_per_r<R>(sum, red);
+        if (threadIdx.x < R) a.partial[(int64_t)blockIdx.x * R + threadIdx.x] = tot;
+        if (FIRST) {
+            c128 tot0 = block_reduce_per_r<R>(sum0, red);
+            if (threadIdx.x < R) a.partial0[(int64_t)blockIdx.x * R + threadIdx.x] = tot0;
+        }
+    }
+}
+
+// Fixed-order final sum of the per-block partials (a8): one warp per (moment m, vector r).
+// partials [M][B][R]  ->  mu[r*mu_rstride + m]
+__global__ void kg_reduce_partials(const c128 *__restrict__ partials, int M, int B, int R,
+                                   c128 *__restrict__ mu, int64_t mu_rstride)
+{
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (warp >= M * R) return;
+    const int m = warp / R, r = warp % R;
+    const c128 *p = partials + (int64_t)m * B * R + r;
+    double sx = 0.0, sy = 0.0;
+    for (int b = lane; b < B; b += 32) {
+        const c128 v = p[(int64_t)b * R];
+        sx += v.x; sy += v.y;
+    }
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) {
+        sx += __shfl_xor_sync(0xffffffffu, sx, off);
+        sy += __shfl_xor_sync(0xffffffffu, sy, off);
+    }
+    if (lane == 0) mu[(int64_t)r * mu_rstride + m] = make_double2(sx, sy);
+}
+
+// dst[i*ld_dst + c] = src[i*ld_src + c], c < ncols (column-block copy between [n][ld] layouts)
+__global__ void kg_copy_cols(const c128 *__restrict__ src, int ld_src, c128 *__restrict__ dst,
+                             int ld_dst, int ncols, int64_t n)
+{
+    const int64_t total = n * ncols;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total;
+         e += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t i = e / ncols;
+        const int c = (int)(e - i * ncols);
+        dst[i * ld_dst + c] = src[i * ld_src + c];
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// create: validate + scale (a1).  flags[0] bit0: index out of range, bit1: nn out of range,
+// bit2: non-finite value, bit3: asymmetric H.  gersh[0] = max_i (|H_ii - E0| + sum_k |H_ik|)
+// as an ordered-int encoded double (all values >= 0 so the bit pattern is monotone).
+// ---------------------------------------------------------------------------------------
+__global__ void kg_build_matrix(int64_t n, int64_t ns, int kmax, const int32_t *__restrict__ nn,
+                                const int32_t *__restrict__ nl_in, const double *__restrict__ hop_in,
+                                const double *__restrict__ onsite_in, const double *__restrict__ x,
+                                double period, double e0, double s, int32_t *__restrict__ nl,
+                                double *__restrict__ hop, double *__restrict__ xhop,
+                                double *__restrict__ onsite, unsigned int *flags,
+                                unsigned long long *gersh)
+{
+    unsigned int bad = 0;
+    double gmax = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < ns;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        if (i >= n) {   // padding rows of the stride
+            for (int k = 0; k < kmax; ++k) { nl[k * ns + i] = 0; hop[k * ns + i] = 0.0; xhop[k * ns + i] = 0.0; }
+            onsite[i] = 0.0;
+            continue;
+        }
+        int cnt = nn[i];
+        if (cnt < 0 || cnt > kmax) { bad |= 2u; cnt = 0; }
+        const double xi = x[i];
+        if (!isfinite(xi)) bad |= 4u;
+        const double eps = onsite_in ? onsite_in[i] : 0.0;
+        if (!isfinite(eps)) bad |= 4u;
+        double g = fabs(eps - e0);
+        onsite[i] = (eps - e0) / s;
+        for (int k = 0; k < kmax; ++k) {
+            int32_t m = (int32_t)i;
+            double h = 0.0, w = 0.0;
+            if (k < cnt) {
+                m = nl_in[k * n + i];
+                h = hop_in[k * n + i];
+                if (m < 0 || m >= n) { bad |= 1u; m = (int32_t)i; h = 0.0; }
+                if (!isfinite(h)) { bad |= 4u; h = 0.0; }
+                double d = x[m] - xi;                       // Delta = X_m - X_i, minimum image
+                if (period > 0.0) {
+                    if (d > 0.5 * period) d -= period;
+                    if (d < -0.5 * period) d += period;
+                }
+                w = (-d) * h / s;                           // (X_i - X_m) H_im / s
+                g += fabs(h);
+                if (m != i) {                               // symmetry: H_mi must equal H_im
+                    bool found = false;
+                    int cm = nn[m];
+                    if (cm < 0 || cm > kmax) cm = 0;
+                    for (int q = 0; q < cm; ++q)
+                        if (nl_in[q * n + m] == (int32_t)i && hop_in[q * n + m] == h) found = true;
+                    if (!found) bad |= 8u;
+                } else {
+                    bad |= 8u;                              // diagonal belongs in onsite_eV
+                }
+            }
+            nl[k * ns + i] = m;
+            hop[k * ns + i] = h / s;
+            xhop[k * ns + i] = w;
+        }
+        gmax = fmax(gmax, g);
+    }
+    if (bad) atomicOr(flags, bad);
+    atomicMax(gersh, (unsigned long long)__double_as_longlong(gmax));
+}
+
+// CSR -> k-major list (rows become columns of the ELL slabs)
+__global__ void kg_csr_to_ell(int64_t n, const int64_t *__restrict__ rowptr,
+                              const int32_t *__restrict__ col, const double *__restrict__ val,
+                              int kmax, int32_t *__restrict__ nn, int32_t *__restrict__ nl,
+                              double *__restrict__ hop)
+{
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t b = rowptr[i], e = rowptr[i + 1];
+        int cnt = (int)(e - b);
+        if (cnt < 0) cnt = -1;           // flagged as bad nn by kg_build_matrix
+        if (cnt > kmax) cnt = kmax + 1;
+        nn[i] = cnt;
+        for (int k = 0; k < kmax; ++k) {
+            const bool ok = cnt >= 0 && k < cnt && k < kmax;
+            nl[(int64_t)k * n + i] = ok ? col[b + k] : (int32_t)i;
+            hop[(int64_t)k * n + i] = ok ? val[b + k] : 0.0;
+        }
+    }
+}
+
+__global__ void kg_csr_max_row(int64_t n, const int64_t *__restrict__ rowptr, int *maxrow, unsigned int *flags)
+{
+    int mx = 0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t c = rowptr[i + 1] - rowptr[i];
+        if (c < 0 || c > 32) atomicOr(flags, 2u);
+        else mx = max(mx, (int)c);
+    }
+    atomicMax(maxrow, mx);
+}

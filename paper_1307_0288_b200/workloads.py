@@ -7,7 +7,7 @@ vectors, following the paper's lattice conventions (N_x dimer 
 zigzag, N_y zigzag chains along armchair, a = 0.142 nm, L_x = sqrt(3) N_x a / 2,
 L_y = 3 N_y a / 2), its hopping (eq 13: -gamma_0, gamma_0 = 2.7 eV) and its vacancy
 model.  The recipe (counter PRNG, site numbering, neighbour order, vacancy
-selection) is stated in DESIGN.md "Input recipe"; oracle/kgo.c implements the same recipe
+selection) is stated in DESIGN.md "Input recipe"; the test oracle implements the same recipe
 independently in C and tests/test_generators.py compares the two bit for bit.
 
 numpy, vectorised (a 16 M-site sheet takes a few seconds).
