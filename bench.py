@@ -1,0 +1,349 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the Chebyshev hot path (arXiv 1307.0288) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl b200|reference]
+
+One STEP = one pass of the whole hot path on the
+BASELINE.json roofline configuration (config 4: 1000x1000 cells = 4,000,000 sites, Anderson
+disorder W = |t|, 1 random-phase vector, M = 3000 moments, dt = 4 hbar/|t| => N_p = 42):
+
+    kg_dos_moments(M)  +  kg_vac(M, n_steps = T)  +  kg_msd(M, n_steps = T)        (T = 1)
+
+i.e. DOS moments, then the first T of the config's 100 correlation-time steps of the
+Green-Kubo (VAC) and Einstein (MSD) loops.  Every time step of those loops does identical
+work (2 evolutions + M-1 fused recursion+dot kernels), so the RATE (Gsite-updates/s) does not
+depend on T; T = 1 keeps the default run within minutes.  `--time-steps 100` runs the full job.
+
+Metric: Gsite-updates/s.  One site-update = one output element of H~ phi in one Chebyshev
+step for one vector; a pair-commutator launch (a2+a6) counts as two.
+
+N > 1 (torchrun): replicas only — the path does not shard (BASELINE.json: "no sharding, no
+inter-GPU collectives").  Each rank runs the same step on its own random vector (the paper
+averages 10-100 independent vectors, eq 21); the only exchange is the final average of
+the [M] moment arrays (a few KB).  Weak scaling.
+
+The JSON line carries `roofline` (dominant kernel, measured live with CUDA events on the
+launching stream) and `cpu_baseline` (the oracle, as it stands, timed on the host cores on a
+bounded sample of the same workload).  `--impl reference` times the oracle only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "Gsite-updates/s (H~.phi per Chebyshev step, fp64 complex)"
+UNIT = "Gsite-updates/s"
+
+# algorithmic bytes per site-update of the dominant kernel (fused recursion + moment dot,
+# general ELL, K = 3): 48 (T_m, T_{m-1}, T_{m+1}) + 16 (phi_L) + (12 idx + 24 hop + 8 onsite)/R
+# -- SURVEY.md 8(d), DESIGN.md "Roofline".
+def mom_bytes_per_update(R: int, kmax: int = 3) -> float:
+    return 48.0 + 16.0 + (kmax * 12.0 + 8.0) / R
+
+
+def site_updates(n: int, R: int, M: int, nt: int, n_p: int) -> dict:
+    """H~-applications of one step, per SURVEY 8(a) a7 (the method's count; both arms use it)."""
+    dos = M - 1
+    vac = 1 + (nt + 1) * (1 + (M - 1)) + nt * 2 * (n_p - 1)
+    msd = (nt + 1) * (M - 1) + nt * 2 * (n_p - 1)
+    per_vec = {"dos": dos, "vac": vac, "msd": msd}
+    return {k: v * n * R for k, v in per_vec.items()}
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(key: str):
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full summary."""
+    p = os.path.join(ROOT, "profiles", "traffic.txt")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        for line in f:
+            parts = line.split("#")[0].split()
+            if len(parts) >= 2 and parts[0] == key:
+                return float(parts[1])
+    return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc = index, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE,
+                stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None,
+                "sm_max_mhz": max(mx) if mx else None, "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+# --------------------------------------------------------------------------------------
+# oracle legs (cpu_baseline, --impl reference): the only places bench.py executes oracle/
+# --------------------------------------------------------------------------------------
+ORACLE_SAMPLE = {"dos_M": 33, "corr_M": 2, "nt": 1}
+
+
+def oracle_step(cfg, olat, phi, sample):
+    """One bounded sample of the step on the host, single-threaded oracle."""
+    from oracle import kgo
+    kgo.dos_moments(olat, cfg.e0, cfg.scale, phi, sample["dos_M"])
+    kgo.vac(olat, cfg.xcoord, cfg.period, cfg.e0, cfg.scale, phi, sample["corr_M"], sample["nt"], cfg.dt_fs)
+    kgo.msd(olat, cfg.xcoord, cfg.period, cfg.e0, cfg.scale, phi, sample["corr_M"], sample["nt"], cfg.dt_fs)
+
+
+def oracle_units(cfg, sample):
+    from oracle import kgo
+    n_p = kgo.bessel_np(cfg.scale * cfg.dt_fs / 0.6582119569)
+    n = cfg.lattice.n
+    d = site_updates(n, 1, sample["dos_M"], 0, n_p)["dos"]
+    c = site_updates(n, 1, sample["corr_M"], sample["nt"], n_p)
+    return d + c["vac"] + c["msd"]
+
+
+def oracle_inputs(cfg):
+    from oracle import kgo
+    from paper_1307_0288_b200 import workloads as W
+    kgo.build()
+    lat = cfg.lattice
+    olat = kgo.Lattice(lat.n, lat.kmax, lat.nn, lat.nl, lat.hop, lat.onsite, lat.x, lat.y,
+                       lat.period_x, lat.period_y)
+    phi = W.random_phase_vectors(lat.n, 1, cfg.seed)[:, 0].copy()
+    return olat, phi
+
+
+def sample_text(cfg, sample):
+    return (f"{cfg.name} lattice ({cfg.lattice.n} sites), 1 vector: dos M={sample['dos_M']}; vac and msd "
+            f"M={sample['corr_M']}, {sample['nt']} time step (dt = 4 hbar/|t|, N_p = 42); "
+            "site-updates counted as in the GPU arm")
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    olat, phi = oracle_inputs(cfg)
+    units = oracle_units(cfg, ORACLE_SAMPLE)
+    for _ in range(args.warmup):
+        oracle_step(cfg, olat, phi, ORACLE_SAMPLE)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_step(cfg, olat, phi, ORACLE_SAMPLE)
+    dt = time.perf_counter() - t0
+    val = units * args.steps / dt / 1e9
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "c128 (fp64 complex)",
+            "data": "synthetic", "config": workload_config(cfg, args, 1),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle",
+                             "sample": sample_text(cfg, ORACLE_SAMPLE)},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(cfg, args, n_ranks):
+    return {"workload": f"BASELINE.json configs[{args.config - 1}] ({cfg.name}): {cfg.lattice.n} sites, "
+                        f"R={cfg.R} vector(s) per GPU, M={cfg.M}, dt={cfg.dt_fs:.6g} fs; step = kg_dos_moments + "
+                        f"kg_vac + kg_msd with {args.time_steps} of the config's {cfg.n_steps} time steps",
+            "sites": cfg.lattice.n, "R": cfg.R, "M": cfg.M, "time_steps": args.time_steps,
+            "parallelism": f"replicas x{n_ranks} (independent random vectors, no data-path collective)",
+            "l2": "inputs larger than L2 (368 MB streamed per Chebyshev step vs 126 MB L2); no flush"}
+
+
+# --------------------------------------------------------------------------------------
+# B200 arm
+# --------------------------------------------------------------------------------------
+def run_b200(args, cfg):
+    import numpy as np
+    import torch
+    from paper_1307_0288_b200 import binding as B
+    from paper_1307_0288_b200 import replicas
+    from paper_1307_0288_b200 import workloads as W
+
+    ctx = replicas.init_from_env("nccl")
+    rank, world, local = ctx.rank, ctx.world, ctx.local_rank
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    lat = cfg.lattice
+    n, R, M, nt = lat.n, cfg.R, cfg.M, args.time_steps
+    h = B.from_lattice(lat, cfg.xcoord, cfg.period, cfg.e0, cfg.scale)
+    n_p, _ = B.bessel_terms(cfg.scale * cfg.dt_fs / W.HBAR)
+    units = site_updates(n, R, M, nt, n_p)
+    units_step = sum(units.values())
+
+    # each rank its own random vectors (streams 16 + rank*R + r of the config's seed)
+    own = replicas.vector_streams(rank, R)
+    phi_np = W.random_phase_vectors(n, own.stop, cfg.seed)[:, own.start:own.stop].copy()
+    phi_dev = torch.from_numpy(phi_np).cuda()
+    mu_dos = torch.empty((R, M), dtype=torch.complex128, device="cuda")
+    mu_vac = torch.empty((R, nt + 1, M), dtype=torch.complex128, device="cuda")
+    mu_msd = torch.empty((R, nt + 1, M), dtype=torch.complex128, device="cuda")
+    # end-to-end leg: pinned HOST buffers through the same C-ABI calls
+    phi_host = torch.from_numpy(phi_np).pin_memory()
+    mu_dos_h = torch.empty((R, M), dtype=torch.complex128).pin_memory()
+    mu_vac_h = torch.empty((R, nt + 1, M), dtype=torch.complex128).pin_memory()
+    mu_msd_h = torch.empty((R, nt + 1, M), dtype=torch.complex128).pin_memory()
+    h2d = 3 * phi_host.numel() * 16
+    d2h = (mu_dos_h.numel() + mu_vac_h.numel() + mu_msd_h.numel()) * 16
+
+    def step_dev():
+        B.dos_moments(h, phi_dev, M, mu=mu_dos)
+        B.vac(h, phi_dev, M, nt, cfg.dt_fs, mu=mu_vac)
+        B.msd(h, phi_dev, M, nt, cfg.dt_fs, mu=mu_msd)
+
+    def step_host():
+        B.dos_moments(h, phi_host, M, mu=mu_dos_h)
+        B.vac(h, phi_host, M, nt, cfg.dt_fs, mu=mu_vac_h)
+        B.msd(h, phi_host, M, nt, cfg.dt_fs, mu=mu_msd_h)
+
+    stream = torch.cuda.current_stream()
+
+    def timed(fn, k):
+        """K steps bracketed by barrier + synchronize; device time by CUDA events on the launching
+        stream; max over ranks."""
+        torch.cuda.synchronize(); ctx.barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = h.launch_count
+        e0.record(stream)
+        for _ in range(k):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize(); ctx.barrier()
+        return ctx.max_over_ranks(e0.elapsed_time(e1)), h.launch_count - l0
+
+    for _ in range(args.warmup):
+        step_dev()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ms, launches = timed(step_dev, args.steps)
+    clocks = sampler.stop() if rank == 0 else None
+    for _ in range(max(1, min(args.warmup, 1))):
+        step_host()
+    ms_e2e, _ = timed(step_host, args.steps)
+
+    # trace average over the replicas' random vectors (eq 21): the only exchange
+    mu_avg = ctx.mean_over_ranks(mu_dos.mean(dim=0))
+    mu0 = complex(mu_avg[0].item())
+
+    # dominant kernel: fused recursion + dot (MODE_MOM, not FIRST).  kg_dos_moments(M) is M-2 such
+    # launches + 1 first-step launch of the same shape + 1 tiny reduction; average launch time =
+    # event time / (M-1) (the reduction is < 0.1 % of the call).
+    reps = 3
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(reps):
+        B.dos_moments(h, phi_dev, M, mu=mu_dos)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    kern_us = e0.elapsed_time(e1) * 1e3 / (reps * (M - 1))
+    peak, peak_src = peaks()
+    bytes_launch = mom_bytes_per_update(R, lat.kmax) * n * R
+    achieved = bytes_launch / (kern_us * 1e-6) / 1e9
+    traffic = ncu_traffic(f"{cfg.name}_mom_R{R}")
+    roofline = {"bound": "hbm", "kernel": f"kg_step_kernel<R={R}, MODE_MOM> (fused T_m+1 = 2H~T_m - T_m-1 + <phi_L|T_m+1>)",
+                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0,
+                "algorithmic_bytes_per_launch": bytes_launch, "us_per_launch": kern_us,
+                "gsu_per_s": n * R / (kern_us * 1e-6) / 1e9, "traffic": traffic}
+
+    if rank != 0:
+        ctx.finalize()
+        return
+    value = units_step * world * args.steps / (ms * 1e-3) / 1e9
+    e2e = units_step * world * args.steps / (ms_e2e * 1e-3) / 1e9
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "c128 (fp64 complex)", "data": "synthetic",
+            "config": workload_config(cfg, args, world),
+            "site_updates_per_step_per_gpu": units, "n_p": n_p, "mu0_trace_average": [mu0.real, mu0.imag],
+            "clocks": clocks,
+            "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "ms_per_step": ms_e2e / args.steps},
+            "gpu_launches": int(launches),
+            "roofline": roofline}
+    if world == 1 and not args.no_cpu_baseline:
+        olat, phi1 = oracle_inputs(cfg)
+        sample = {"dos_M": 65, "corr_M": 4, "nt": 1}
+        t0 = time.perf_counter()
+        oracle_step(cfg, olat, phi1, sample)
+        dt = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": oracle_units(cfg, sample) / dt / 1e9, "unit": UNIT, "cores": 1,
+                                "kind": "oracle", "seconds": dt, "host_cores_available": os.cpu_count(),
+                                "sample": sample_text(cfg, sample)}
+    print(json.dumps(line), flush=True)
+    ctx.finalize()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index 1..5 (default 4, the roofline config)")
+    ap.add_argument("--time-steps", type=int, default=1, help="correlation-time steps of kg_vac / kg_msd per bench step")
+    ap.add_argument("--shrink", type=int, default=1, help="divide the lattice's linear size (debug only)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "b200":
+        print("note: warmup < 3 violates the timing rules; use only for debugging", file=sys.stderr)
+    from paper_1307_0288_b200 import workloads as W
+    cfg = W.make_config(args.config, shrink=args.shrink)
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_b200(args, cfg)
+
+
+if __name__ == "__main__":
+    main()
