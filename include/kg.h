@@ -176,7 +176,12 @@ int kg_bessel_terms(double x, double bessel_eps, int *np_out, double *j, int cap
 enum {
     KG_OPT_USE_GRAPHS = 1,   /* 1 (default): replay the moment loop as a CUDA graph */
     KG_OPT_BLOCKS_PER_SM = 2, /* persistent grid = SMs * this (default chosen per kernel) */
-    KG_OPT_THREADS = 3       /* threads per block (default 256) */
+    KG_OPT_THREADS = 3,      /* threads per block (default 256) */
+    KG_OPT_STAGED = 4,       /* 1 (default): moment steps run the TMA-staged kernel when eligible */
+    KG_OPT_STAGES = 5,       /* shared-memory ring depth of the staged kernel (0 = auto) */
+    KG_OPT_STAGED_CTAS = 6,  /* CTAs per SM of the staged kernel (0 = auto) */
+    KG_OPT_ALTERNATE = 7,    /* 1 (default): alternate the sweep direction step to step (L2 reuse) */
+    KG_OPT_DICT = 8          /* 0: drop the hopping dictionary, stream fp64 hoppings (general path) */
 };
 int kg_set_option(kg_hamiltonian *h, int option, int64_t value);
 

@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 SRC = [os.path.join(HERE, "csrc", "kg.cu")]
-DEPS = SRC + [os.path.join(HERE, "csrc", "kg_kernels.cuh"), os.path.join(ROOT, "include", "kg.h")]
+DEPS = SRC + [os.path.join(HERE, "csrc", "kg_kernels.cuh"), os.path.join(HERE, "csrc", "kg_staged.cuh"), os.path.join(ROOT, "include", "kg.h")]
 LIB = os.path.join(HERE, "libkg.so")
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

@@ -3,7 +3,9 @@
 // O(N_p) series coefficients (Bessel functions, eq 36) on the host and enqueues kernels.
 #include "kg.h"
 #include "kg_kernels.cuh"
+#include "kg_staged.cuh"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -59,7 +61,11 @@ struct kg_hamiltonian {
     double s, e0, period;
     bool has_onsite;
     int32_t *nl;
+    int32_t *nlp;             // (dictionary id << 28) | NL_ik, for the staged kernel (DICT)
     double *hop, *xhop, *onsite;
+    double dict[16];          // hopping dictionary, dict[0] = 0
+    int ndict;                // entries in use (0: hoppings do not fit a dictionary)
+    int staged, stages, staged_ctas, alternate;   // options of the staged kernel
     void *ws[WS_COUNT];
     size_t ws_bytes[WS_COUNT];
     size_t matrix_bytes;
@@ -172,6 +178,73 @@ static StepArgs base_args(const kg_hamiltonian *h)
     return a;
 }
 
+// ---- staged kernel (kg_staged.cuh): plan + dispatch ----
+struct StagedPlan { bool ok; int grid, nst, ntiles; size_t smem; };
+
+template <int R, bool ONS, bool DICT>
+static cudaError_t staged_launch_t(const kg_hamiltonian *h, const StagedArgs &a, const StagedPlan &p, cudaStream_t st)
+{
+    static size_t configured[64] = {0};
+    const int dev = h->device & 63;
+    if (configured[dev] < p.smem) {
+        cudaError_t e = cudaFuncSetAttribute(kg_mom_staged_kernel<R, ONS, DICT>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem);
+        if (e != cudaSuccess) return e;
+        configured[dev] = p.smem;
+    }
+    kg_mom_staged_kernel<R, ONS, DICT><<<p.grid, SG_THREADS, p.smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+template <int R>
+static cudaError_t staged_launch_r(const kg_hamiltonian *h, const StagedArgs &a, const StagedPlan &p, cudaStream_t st)
+{
+    const bool dict = h->ndict > 0;
+    if (h->has_onsite) return dict ? staged_launch_t<R, true, true>(h, a, p, st) : staged_launch_t<R, true, false>(h, a, p, st);
+    return dict ? staged_launch_t<R, false, true>(h, a, p, st) : staged_launch_t<R, false, false>(h, a, p, st);
+}
+
+static cudaError_t staged_launch(kg_hamiltonian *h, int R, const StagedArgs &a, const StagedPlan &p, cudaStream_t st)
+{
+    h->launches++;
+    switch (R) {
+    case 1: return staged_launch_r<1>(h, a, p, st);
+    case 2: return staged_launch_r<2>(h, a, p, st);
+    case 4: return staged_launch_r<4>(h, a, p, st);
+    case 8: return staged_launch_r<8>(h, a, p, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+static StagedPlan staged_plan(const kg_hamiltonian *h, int R)
+{
+    StagedPlan p;
+    memset(&p, 0, sizeof(p));
+    if (!h->staged || h->kmax != 3 || R > 8) return p;
+    const int cs = SG_TILE_E / R;
+    const size_t stage = ((size_t)SG_TILE_E * 48 + (size_t)cs * 12 + (h->has_onsite ? (size_t)cs * 8 : 0) +
+                          (h->ndict > 0 ? 0 : (size_t)cs * 24) + 127) / 128 * 128;
+    const size_t header = ((size_t)2 * SG_MAX_STAGES * 8 + 128 + (size_t)32 * R * 16 + 127) / 128 * 128;
+    // auto: 3 CTAs per SM with a 2-deep ring measured best on config 4 (profiles/); fewer CTAs
+    // when a stage is too large for that (fp64 hoppings staged)
+    int ctas = h->staged_ctas > 0 ? h->staged_ctas : 3, nst = 0;
+    for (;; --ctas) {
+        const size_t budget = (size_t)228 * 1024 / ctas - 1024;
+        nst = h->stages > 0 ? h->stages : (int)((budget - header) / stage);
+        if (nst >= 2 || h->staged_ctas > 0 || ctas == 1) break;
+    }
+    if (nst > SG_MAX_STAGES) nst = SG_MAX_STAGES;
+    if (nst < 2 || header + (size_t)nst * stage > (size_t)227 * 1024) return p;
+    p.nst = nst;
+    p.smem = header + (size_t)nst * stage;
+    const int64_t nt = (h->n * R + SG_TILE_E - 1) / SG_TILE_E;
+    p.ntiles = (int)nt;
+    const int64_t cap = (int64_t)h->num_sms * ctas;
+    p.grid = (int)(nt < cap ? nt : cap);
+    p.ok = true;
+    return p;
+}
+
 static bool r_ok(int R, bool allow16) { return R == 1 || R == 2 || R == 4 || R == 8 || (allow16 && R == 16); }
 
 // --------------------------------------------------------------------------------------
@@ -255,13 +328,15 @@ static int create_from_device_list(kg_hamiltonian **out, int64_t n, int kmax, co
 {
     kg_hamiltonian *h = new (std::nothrow) kg_hamiltonian();
     if (!h) return fail(KG_ENOMEM, "host allocation failed");
-    h->n = n; h->ns = (n + 31) / 32 * 32; h->kmax = kmax;
+    h->n = n; h->ns = (n + SG_TILE_E - 1) / SG_TILE_E * SG_TILE_E; h->kmax = kmax;
     h->s = s; h->e0 = e0; h->period = period;
-    h->nl = nullptr; h->hop = h->xhop = h->onsite = nullptr;
+    h->nl = h->nlp = nullptr; h->hop = h->xhop = h->onsite = nullptr;
+    h->ndict = 0; h->staged = 1; h->stages = 0; h->staged_ctas = 0; h->alternate = 1;
+    memset(h->dict, 0, sizeof(h->dict));
     memset(h->ws, 0, sizeof(h->ws));
     memset(h->ws_bytes, 0, sizeof(h->ws_bytes));
     h->launches = 0;
-    h->threads = 256; h->blocks_per_sm = 8; h->use_graphs = -1;
+    h->threads = 256; h->blocks_per_sm = 6; h->use_graphs = -1;
     unsigned int *d_flags = nullptr;
     int rc = KG_OK;
     auto cleanup = [&](int code) { if (d_flags) cudaFree(d_flags); kg_destroy_hamiltonian(h); return code; };
@@ -297,6 +372,46 @@ static int create_from_device_list(kg_hamiltonian **out, int64_t n, int kmax, co
         rc = fail(KG_ESPECTRUM, "Gershgorin bound %.6g eV of (H - E0) exceeds scale %.6g eV", gersh, s);
     if (rc) return cleanup(rc);
     h->has_onsite = d_ons != nullptr || e0 != 0.0;
+    // hopping dictionary for the staged kernel: <= 15 distinct non-zero values of H_ik/s
+    if (kmax == 3 && n <= (int64_t)SG_IDX_MASK + 1) {
+        unsigned long long tab[16];
+        for (int q = 0; q < 16; ++q) tab[q] = SG_DICT_EMPTY;
+        tab[15] = 0;   // overflow flag lives in slot 15
+        unsigned long long *d_tab = nullptr;
+        double *d_dict = nullptr;
+        if ((e = cudaMalloc(&d_tab, 16 * 8)) != cudaSuccess || (e = cudaMalloc(&d_dict, 16 * 8)) != cudaSuccess ||
+            (e = cudaMalloc(&h->nlp, slab * 4)) != cudaSuccess) {
+            cudaFree(d_tab); cudaFree(d_dict);
+            return cleanup(fail(KG_ENOMEM, "dictionary allocation: %s", cudaGetErrorString(e)));
+        }
+        h->matrix_bytes += slab * 4;
+        auto cleanup2 = [&](int code) { cudaFree(d_tab); cudaFree(d_dict); return cleanup(code); };
+        if ((e = cudaMemcpyAsync(d_tab, tab, sizeof(tab), cudaMemcpyHostToDevice, st)) != cudaSuccess)
+            return cleanup2(fail(KG_ECUDA, "dictionary: %s", cudaGetErrorString(e)));
+        kg_dict_collect<<<grid, 256, 0, st>>>(h->hop, (int64_t)slab, d_tab, (unsigned int *)(d_tab + 15));
+        h->launches++;
+        if ((e = cudaGetLastError()) != cudaSuccess ||
+            (e = cudaMemcpyAsync(tab, d_tab, sizeof(tab), cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+            (e = cudaStreamSynchronize(st)) != cudaSuccess)
+            return cleanup2(fail(KG_ECUDA, "kg_dict_collect: %s", cudaGetErrorString(e)));
+        if ((unsigned int)tab[15] == 0) {
+            std::vector<double> vals;
+            for (int q = 0; q < 15; ++q)
+                if (tab[q] != SG_DICT_EMPTY) { double v; memcpy(&v, &tab[q], 8); vals.push_back(v); }
+            std::sort(vals.begin(), vals.end());
+            h->ndict = 1 + (int)vals.size();
+            for (size_t q = 0; q < vals.size(); ++q) h->dict[1 + q] = vals[q];
+            if ((e = cudaMemcpyAsync(d_dict, h->dict, 16 * 8, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+                return cleanup2(fail(KG_ECUDA, "dictionary: %s", cudaGetErrorString(e)));
+            kg_dict_pack<<<grid, 256, 0, st>>>(h->nl, h->hop, (int64_t)slab, d_dict, h->ndict, h->nlp);
+            h->launches++;
+            if ((e = cudaGetLastError()) != cudaSuccess || (e = cudaStreamSynchronize(st)) != cudaSuccess)
+                return cleanup2(fail(KG_ECUDA, "kg_dict_pack: %s", cudaGetErrorString(e)));
+        } else {
+            cudaFree(h->nlp); h->nlp = nullptr; h->matrix_bytes -= slab * 4;
+        }
+        cudaFree(d_tab); cudaFree(d_dict);
+    }
     cudaFree(d_flags);
     *out = h;
     return KG_OK;
@@ -398,7 +513,7 @@ extern "C" int kg_destroy_hamiltonian(kg_hamiltonian *h)
 {
     if (!h) return KG_OK;
     for (auto &g : h->graphs) cudaGraphExecDestroy(g.exec);
-    cudaFree(h->nl); cudaFree(h->hop); cudaFree(h->xhop); cudaFree(h->onsite);
+    cudaFree(h->nl); cudaFree(h->nlp); cudaFree(h->hop); cudaFree(h->xhop); cudaFree(h->onsite);
     for (int i = 0; i < WS_COUNT; ++i) cudaFree(h->ws[i]);
     delete h;
     return KG_OK;
@@ -426,6 +541,17 @@ extern "C" int kg_set_option(kg_hamiltonian *h, int option, int64_t value)
     case KG_OPT_THREADS:
         if (value != 64 && value != 128 && value != 256) return fail(KG_EINVAL, "threads must be 64, 128 or 256");
         h->threads = (int)value; break;
+    case KG_OPT_STAGED: h->staged = value != 0; break;
+    case KG_OPT_STAGES:
+        if (value < 0 || value > SG_MAX_STAGES) return fail(KG_EINVAL, "stages must be in [0, %d]", SG_MAX_STAGES);
+        h->stages = (int)value; break;
+    case KG_OPT_STAGED_CTAS:
+        if (value < 0 || value > 8) return fail(KG_EINVAL, "staged CTAs per SM must be in [0, 8]");
+        h->staged_ctas = (int)value; break;
+    case KG_OPT_ALTERNATE: h->alternate = value != 0; break;
+    case KG_OPT_DICT:
+        if (value != 0) return fail(KG_EINVAL, "the dictionary can only be switched off");
+        h->ndict = 0; break;
     default: return fail(KG_EINVAL, "unknown option %d", option);
     }
     for (auto &g : h->graphs) cudaGraphExecDestroy(g.exec);
@@ -439,9 +565,17 @@ extern "C" int kg_set_option(kg_hamiltonian *h, int option, int64_t value)
 
 // enqueue the M-1 fused recursion+dot kernels of Alg. 5 (a2+a3); partials [M][grid][R]
 static int enqueue_moment_steps(kg_hamiltonian *h, const c128 *phiL, int ldL, const c128 *phiR, int ldR,
-                                int R, int M, c128 *ta, c128 *tb, c128 *part, int grid, cudaStream_t st)
+                                int R, int M, c128 *ta, c128 *tb, c128 *part, int grid,
+                                const StagedPlan &sp, cudaStream_t st)
 {
     const size_t prow = (size_t)grid * R;
+    StagedArgs sa;
+    memset(&sa, 0, sizeof(sa));
+    if (sp.ok) {
+        sa.idx = h->ndict > 0 ? h->nlp : h->nl; sa.hop = h->hop; sa.onsite = h->onsite;
+        memcpy(sa.dict, h->dict, sizeof(sa.dict));
+        sa.n = h->n; sa.ns = h->ns; sa.phiL = phiL; sa.ntiles = sp.ntiles; sa.nstages = sp.nst;
+    }
     StepArgs a = base_args(h);
     a.phiL = phiL; a.ld_L = ldL;
     // m = 1: T_1 = H~ T_0, partial rows 0 and 1
@@ -455,7 +589,14 @@ static int enqueue_moment_steps(kg_hamiltonian *h, const c128 *phiL, int ldL, co
         if (m == 2) { a.cur = ta; a.ld_cur = R; a.prev = phiR; a.ld_prev = ldR; a.next = tb; }
         else if (m & 1) { a.cur = tb; a.ld_cur = R; a.prev = ta; a.ld_prev = R; a.next = ta; }
         else { a.cur = ta; a.ld_cur = R; a.prev = tb; a.ld_prev = R; a.next = tb; }
-        CUDA_TRY(launch_step(h, MODE_MOM, false, R, a, grid, st));
+        if (sp.ok && ldL == R && a.ld_cur == R && a.ld_prev == R) {
+            // tuned form of the same step: TMA-staged streams, alternating sweep direction
+            sa.cur = a.cur; sa.prev = a.prev; sa.next = a.next; sa.partial = a.partial;
+            sa.reverse = h->alternate ? (m & 1) : 0;
+            CUDA_TRY(staged_launch(h, R, sa, sp, st));
+        } else {
+            CUDA_TRY(launch_step(h, MODE_MOM, false, R, a, grid, st));
+        }
     }
     return KG_OK;
 }
@@ -473,7 +614,8 @@ static int moments_device(kg_hamiltonian *h, const c128 *phiL, int ldL, const c1
                           int M, c128 *mu, int64_t mu_rstride, cudaStream_t st)
 {
     const int64_t elems = h->n * R;
-    const int grid = grid_for(h, elems);
+    const StagedPlan sp = staged_plan(h, R);
+    const int grid = sp.ok ? sp.grid : grid_for(h, elems);   // one partial row shape for both kernels
     void *ta, *tb, *part;
     int rc;
     if ((rc = ws_get(h, WS_TA, (size_t)elems * 16, &ta)) || (rc = ws_get(h, WS_TB, (size_t)elems * 16, &tb)) ||
@@ -489,7 +631,7 @@ static int moments_device(kg_hamiltonian *h, const c128 *phiL, int ldL, const c1
             cudaGraph_t graph;
             CUDA_TRY(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
             const int64_t before = h->launches;
-            rc = enqueue_moment_steps(h, phiL, ldL, phiR, ldR, R, M, (c128 *)ta, (c128 *)tb, (c128 *)part, grid, st);
+            rc = enqueue_moment_steps(h, phiL, ldL, phiR, ldR, R, M, (c128 *)ta, (c128 *)tb, (c128 *)part, grid, sp, st);
             h->launches = before;
             cudaError_t e = cudaStreamEndCapture(st, &graph);
             if (rc) { if (e == cudaSuccess) cudaGraphDestroy(graph); return rc; }
@@ -503,7 +645,7 @@ static int moments_device(kg_hamiltonian *h, const c128 *phiL, int ldL, const c1
         CUDA_TRY(cudaGraphLaunch(exec, st));
         h->launches += M - 1;
     } else {
-        if ((rc = enqueue_moment_steps(h, phiL, ldL, phiR, ldR, R, M, (c128 *)ta, (c128 *)tb, (c128 *)part, grid, st)))
+        if ((rc = enqueue_moment_steps(h, phiL, ldL, phiR, ldR, R, M, (c128 *)ta, (c128 *)tb, (c128 *)part, grid, sp, st)))
             return rc;
     }
     const int warps = M * R;

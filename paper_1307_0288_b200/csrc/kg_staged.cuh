@@ -1,0 +1,287 @@
+// kg_staged.cuh — the bandwidth-tuned form of the hot kernel (sm_100a): the fused Chebyshev
+// step  T_{m+1} = 2 H~ T_m - T_{m-1}  (eq 38; Alg. 5 l.6 P:363) with the moment inner
+// product <phi_L|T_{m+1}> (Alg. 5 l.7 P:365, eq 46) folded into the same pass.
+//
+// Same arithmetic as kg_step_kernel<MODE_MOM> (kg_kernels.cuh); what differs is how the bytes
+// move:
+//
+//  * every CONTIGUOUS stream of a tile — the tile's own T_m, T_{m-1} and phi_L elements, its
+//    neighbour indices and its on-site energies — is fetched by the TMA engine with 1-D bulk
+//    copies (cp.async.bulk.shared.global, completion on an mbarrier) into a ring of shared-
+//    memory stages, issued by one producer lane several tiles ahead of the consumers.  The
+//    stream loads therefore cost no registers and no warp stalls; DRAM requests stay in
+//    flight independently of occupancy.
+//  * the only loads left in the consumer warps are the GATHERS T_m[NL_ik].  Neighbours that
+//    lie inside the tile are read from the staged copy of T_m in shared memory; the others
+//    (the lattice rows above / below) are 16-byte ld.global.nc hits in L2, brought there by
+//    the neighbouring tiles' streams.
+//  * the matrix stream is compressed when the hoppings allow it (DICT): a hopping that takes
+//    at most 15 distinct non-zero values — one value, -gamma_0/s, in the paper's model, eq 13
+//    is stored as a 4-bit dictionary id in the top bits of the int32 neighbour index
+//    (n <= 2^28), so a row costs 12 B of indices + 8 B on-site instead of 44 B.  Otherwise the
+//    fp64 hoppings are staged like the indices (general Alg. 8 matrix).
+//  * persistent grid, tiles interleaved over the CTAs; the sweep direction alternates from
+//    one Chebyshev step to the next (`reverse`), so that the tail of step m — the last ~L2-size
+//    worth of T_{m+1}, T_m, phi_L and matrix — is what step m+1 touches first and is served
+//    from the 126 MB L2 instead of HBM.
+//
+// Determinism: tile -> CTA -> thread -> element assignment is a pure function of the launch
+// shape; per-thread sums run in a fixed order, the block tree is fixed, kg_reduce_partials
+// adds the per-CTA partials in CTA order.  Moments are bitwise reproducible run to run.
+#pragma once
+#include "kg_kernels.cuh"
+
+#define SG_TILE_E 512          // elements (site, vector) per tile
+#define SG_CONSUMERS 256       // consumer threads; + one producer warp
+#define SG_THREADS (SG_CONSUMERS + 32)
+#define SG_EPT (SG_TILE_E / SG_CONSUMERS)
+#define SG_IDX_MASK 0x0FFFFFFF // DICT: neighbour index in bits 0..27, dictionary id in 28..31
+#define SG_MAX_STAGES 8
+
+struct StagedArgs {
+    const int32_t *idx;    // [3][ns]  DICT: (id << 28) | NL_ik ; else NL_ik
+    const double *hop;     // [3][ns]  H_ik / s              (used when !DICT)
+    const double *onsite;  // [ns]     (H_ii - E0)/s         (used when ONS)
+    double dict[16];       // DICT: hopping value per id, dict[0] = 0
+    int64_t n, ns;
+    const c128 *cur;       // T_m      [n][R]
+    const c128 *prev;      // T_{m-1}  [n][R]
+    c128 *next;            // T_{m+1}  [n][R]; may alias prev
+    const c128 *phiL;      // [n][R]
+    c128 *partial;         // [grid][R]
+    int ntiles;
+    int reverse;           // sweep the tiles from the last to the first
+    int nstages;
+};
+
+__device__ __forceinline__ uint32_t sg_smem_u32(const void *p)
+{
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void sg_mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void sg_mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void sg_mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ bool sg_mbar_try_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void sg_mbar_wait(uint32_t bar, uint32_t parity)
+{
+    while (!sg_mbar_try_wait(bar, parity)) {}
+}
+// 1-D bulk copy global -> shared through the TMA engine; bytes % 16 == 0, 16-byte aligned ends
+__device__ __forceinline__ void sg_bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+
+// byte offsets inside one stage
+template <int R, bool ONS, bool DICT>
+struct SgLayout {
+    static constexpr int CS = SG_TILE_E / R;                 // sites per tile
+    static constexpr int OFF_SELF = 0;
+    static constexpr int OFF_PREV = OFF_SELF + SG_TILE_E * 16;
+    static constexpr int OFF_PHIL = OFF_PREV + SG_TILE_E * 16;
+    static constexpr int OFF_IDX = OFF_PHIL + SG_TILE_E * 16;
+    static constexpr int OFF_ONS = OFF_IDX + 3 * CS * 4;
+    static constexpr int OFF_HOP = OFF_ONS + (ONS ? CS * 8 : 0);
+    static constexpr int STAGE = (OFF_HOP + (DICT ? 0 : 3 * CS * 8) + 127) / 128 * 128;
+    // header: full[8], empty[8] mbarriers, dict[16], reduction scratch [32][R] c128
+    static constexpr int OFF_DICT = 2 * SG_MAX_STAGES * 8;
+    static constexpr int OFF_RED = OFF_DICT + 16 * 8;
+    static constexpr int HEADER = (OFF_RED + 32 * R * 16 + 127) / 128 * 128;
+};
+
+template <int R, bool ONS, bool DICT>
+__global__ void __launch_bounds__(SG_THREADS) kg_mom_staged_kernel(const StagedArgs a)
+{
+    typedef SgLayout<R, ONS, DICT> L;
+    constexpr int CS = L::CS;
+    extern __shared__ __align__(128) unsigned char sg_smem[];
+    uint64_t *bars = reinterpret_cast<uint64_t *>(sg_smem);
+    double *dict_s = reinterpret_cast<double *>(sg_smem + L::OFF_DICT);
+    c128 *red = reinterpret_cast<c128 *>(sg_smem + L::OFF_RED);
+    unsigned char *stages = sg_smem + L::HEADER;
+
+    const int tid = threadIdx.x;
+    const int nst = a.nstages;
+    const uint32_t full0 = sg_smem_u32(bars), empty0 = sg_smem_u32(bars + SG_MAX_STAGES);
+    if (tid == 0) {
+        for (int s = 0; s < nst; ++s) {
+            sg_mbar_init(full0 + 8 * s, 1);
+            sg_mbar_init(empty0 + 8 * s, SG_CONSUMERS / 32);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (DICT && tid < 16) dict_s[tid] = a.dict[tid];
+    __syncthreads();
+
+    const int64_t total = a.n * R;
+    const int my_tiles = ((int)blockIdx.x < a.ntiles) ? (a.ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
+    c128 sum = make_double2(0.0, 0.0);
+
+    if (tid >= SG_CONSUMERS) {
+        // ---------------- producer warp: one lane feeds the ring ----------------
+        if (tid == SG_CONSUMERS) {
+            for (int j = 0; j < my_tiles; ++j) {
+                const int s = j % nst;
+                const uint32_t ph = (uint32_t)(j / nst) & 1u;
+                int t = (int)blockIdx.x + j * (int)gridDim.x;
+                if (a.reverse) t = a.ntiles - 1 - t;
+                const int64_t site0 = (int64_t)t * CS, e0 = site0 * R;
+                const int64_t rem = total - e0;
+                const uint32_t vbytes = (uint32_t)(rem < SG_TILE_E ? rem : SG_TILE_E) * 16u;
+                const uint32_t full = full0 + 8 * s;
+                sg_mbar_wait(empty0 + 8 * s, ph ^ 1u);
+                const uint32_t sb = sg_smem_u32(stages + (size_t)s * L::STAGE);
+                uint32_t tx = 3u * vbytes + 3u * CS * 4u;
+                if (ONS) tx += CS * 8u;
+                if (!DICT) tx += 3u * CS * 8u;
+                sg_mbar_expect_tx(full, tx);
+                sg_bulk_g2s(sb + L::OFF_SELF, a.cur + e0, vbytes, full);
+                sg_bulk_g2s(sb + L::OFF_PREV, a.prev + e0, vbytes, full);
+                sg_bulk_g2s(sb + L::OFF_PHIL, a.phiL + e0, vbytes, full);
+#pragma unroll
+                for (int k = 0; k < 3; ++k)
+                    sg_bulk_g2s(sb + L::OFF_IDX + k * CS * 4, a.idx + k * a.ns + site0, CS * 4u, full);
+                if (ONS) sg_bulk_g2s(sb + L::OFF_ONS, a.onsite + site0, CS * 8u, full);
+                if (!DICT) {
+#pragma unroll
+                    for (int k = 0; k < 3; ++k)
+                        sg_bulk_g2s(sb + L::OFF_HOP + k * CS * 8, a.hop + k * a.ns + site0, CS * 8u, full);
+                }
+            }
+        }
+    } else {
+        // ---------------- consumers: gathers + arithmetic ----------------
+        const int r = tid & (R - 1);
+        for (int j = 0; j < my_tiles; ++j) {
+            const int s = j % nst;
+            const uint32_t ph = (uint32_t)(j / nst) & 1u;
+            int t = (int)blockIdx.x + j * (int)gridDim.x;
+            if (a.reverse) t = a.ntiles - 1 - t;
+            const int64_t site0 = (int64_t)t * CS, e0 = site0 * R;
+            const int64_t rem = total - e0;
+            const int ne = (int)(rem < SG_TILE_E ? rem : SG_TILE_E);
+            const unsigned char *sb = stages + (size_t)s * L::STAGE;
+            const c128 *self_s = reinterpret_cast<const c128 *>(sb + L::OFF_SELF);
+            const c128 *prev_s = reinterpret_cast<const c128 *>(sb + L::OFF_PREV);
+            const c128 *phil_s = reinterpret_cast<const c128 *>(sb + L::OFF_PHIL);
+            const int32_t *idx_s = reinterpret_cast<const int32_t *>(sb + L::OFF_IDX);
+            const double *ons_s = reinterpret_cast<const double *>(sb + L::OFF_ONS);
+            const double *hop_s = reinterpret_cast<const double *>(sb + L::OFF_HOP);
+            sg_mbar_wait(full0 + 8 * s, ph);
+
+            c128 v[SG_EPT][3];
+            double hk[SG_EPT][3];
+#pragma unroll
+            for (int q = 0; q < SG_EPT; ++q) {
+                const int le = tid + q * SG_CONSUMERS;
+                const int ls = le / R;
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    const int32_t w = idx_s[k * CS + ls];
+                    int64_t m;
+                    if (DICT) {
+                        m = w & SG_IDX_MASK;
+                        hk[q][k] = dict_s[(uint32_t)w >> 28];
+                    } else {
+                        m = w;
+                        hk[q][k] = hop_s[k * CS + ls];
+                    }
+                    const int64_t d = m - site0;
+                    if ((uint64_t)d < (uint64_t)CS) v[q][k] = self_s[(int)d * R + r];
+                    else v[q][k] = ld_nc(a.cur + m * R + r);
+                }
+            }
+#pragma unroll
+            for (int q = 0; q < SG_EPT; ++q) {
+                const int le = tid + q * SG_CONSUMERS;
+                const int ls = le / R;
+                c128 acc = make_double2(0.0, 0.0);
+                if (ONS) {
+                    const double eps = ons_s[ls];
+                    const c128 self = self_s[le];
+                    acc.x = eps * self.x; acc.y = eps * self.y;
+                }
+#pragma unroll
+                for (int k = 0; k < 3; ++k) cfma_r(acc, hk[q][k], v[q][k]);
+                if (le < ne) {
+                    const c128 p = prev_s[le];
+                    const c128 tt = make_double2(fma(2.0, acc.x, -p.x), fma(2.0, acc.y, -p.y));
+                    a.next[e0 + le] = tt;
+                    const c128 Lv = phil_s[le];
+                    sum.x = fma(Lv.x, tt.x, fma(Lv.y, tt.y, sum.x));      // conj(L) * t
+                    sum.y = fma(Lv.x, tt.y, fma(-Lv.y, tt.x, sum.y));
+                }
+            }
+            __syncwarp();
+            if ((tid & 31) == 0) sg_mbar_arrive(empty0 + 8 * s);
+        }
+    }
+    // block total per vector r (the producer warp adds zeros)
+    c128 tot = block_reduce_per_r<R>(sum, red);
+    if (tid < R) a.partial[(int64_t)blockIdx.x * R + tid] = tot;
+}
+
+// ---------------------------------------------------------------------------------------
+// create: hopping dictionary.  table[0..14] = bit patterns of the distinct non-zero values
+// of H_ik/s found so far (EMPTY = all ones, a NaN pattern no finite hopping has).
+// ---------------------------------------------------------------------------------------
+#define SG_DICT_EMPTY 0xFFFFFFFFFFFFFFFFull
+
+__global__ void kg_dict_collect(const double *__restrict__ hop, int64_t count,
+                                unsigned long long *table, unsigned int *overflow)
+{
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < count;
+         e += (int64_t)gridDim.x * blockDim.x) {
+        const double h = hop[e];
+        if (h == 0.0) continue;
+        const unsigned long long bits = (unsigned long long)__double_as_longlong(h);
+        bool found = false;
+        for (int sl = 0; sl < 15 && !found; ++sl) {
+            unsigned long long c = *((volatile unsigned long long *)table + sl);
+            if (c == SG_DICT_EMPTY) {
+                const unsigned long long old = atomicCAS(table + sl, SG_DICT_EMPTY, bits);
+                c = (old == SG_DICT_EMPTY) ? bits : old;
+            }
+            found = (c == bits);
+        }
+        if (!found) atomicOr(overflow, 1u);
+    }
+}
+
+// idx[e] = (id << 28) | nl[e], id = position of hop[e] in the sorted dictionary (0 for 0.0)
+__global__ void kg_dict_pack(const int32_t *__restrict__ nl, const double *__restrict__ hop,
+                             int64_t count, const double *__restrict__ dict, int ndict,
+                             int32_t *__restrict__ idx)
+{
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < count;
+         e += (int64_t)gridDim.x * blockDim.x) {
+        const double h = hop[e];
+        uint32_t id = 0;
+        if (h != 0.0)
+            for (int q = 1; q < ndict; ++q)
+                if (dict[q] == h) id = (uint32_t)q;
+        idx[e] = (int32_t)((id << 28) | (uint32_t)nl[e]);
+    }
+}

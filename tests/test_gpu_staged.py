@@ -1,0 +1,136 @@
+"""GPU parity of the TMA-staged moment kernel (csrc/kg_staged.cuh) against the CPU oracle.
+
+The staged kernel is the default for the recursion+dot steps (kmax = 3, contiguous vectors);
+these cases pin down what is specific to it: the hopping dictionary (one value, a few values,
+too many values -> fp64 hoppings staged), the ring of stages wrapping several times per CTA,
+the alternating sweep direction, ragged last tile, every R, and bitwise agreement of repeated
+runs.  Tolerance as in test_gpu_parity.py (BASELINE.json: <= 1e-10 max-norm relative)."""
+import numpy as np
+import pytest
+
+from helpers import relerr, to_oracle_lattice
+from paper_1307_0288_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1307_0288_b200 import binding
+    return binding
+
+
+def dev(x):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def host(t):
+    return t.cpu().numpy()
+
+
+def sheet(ncx, ncy, nvac, onsite, seed=11):
+    full = W.honeycomb(ncx, ncy)
+    lat = W.remove_sites(full, W.vacancy_mask(full.n, nvac, seed)) if nvac else full
+    if onsite:
+        lat.onsite = W.anderson(lat.n, 2.7, seed + 1)
+    return lat
+
+
+def set_hoppings(lat, kind):
+    """Symmetric per-bond hoppings: a function of the unordered pair (i, NL_ik)."""
+    n = lat.n
+    nl = lat.nl.reshape(3, n).astype(np.int64)
+    i = np.arange(n)[None, :]
+    lo, hi = np.minimum(i, nl), np.maximum(i, nl)
+    if kind == "three":
+        vals = np.array([-2.7, -2.5, -3.0])
+        hop = vals[(lo + hi) % 3]
+    else:   # "many": a different value on (almost) every bond
+        hop = -2.7 * (1.0 + 0.1 * np.sin(12.9898 * lo + 78.233 * hi))
+    used = np.arange(3)[:, None] < lat.nn[None, :]
+    lat.hop = np.where(used, hop, 0.0).reshape(-1)
+    return lat
+
+
+def scale_for(lat):
+    return (3 * 3.0 + (1.35 if lat.onsite is not None else 0.0)) * 1.05
+
+
+@pytest.mark.parametrize("R", [1, 2, 4, 8])
+@pytest.mark.parametrize("kind", ["uniform", "three", "many"])
+@pytest.mark.parametrize("onsite", [False, True])
+def test_staged_moments_hopping_kinds(B, kgo, R, kind, onsite):
+    lat = sheet(17, 13, 41, onsite)        # 884 - 41 = 843 sites: ragged last tile for every R
+    if kind != "uniform":
+        lat = set_hoppings(lat, kind)
+    s = scale_for(lat)
+    olat = to_oracle_lattice(kgo, lat)
+    h = B.from_lattice(lat, lat.x, lat.period_x, 0.0, s)
+    phi = W.random_phase_vectors(lat.n, R, 3)
+    rng = np.random.default_rng(R)
+    L = rng.normal(size=(lat.n, R)) + 1j * rng.normal(size=(lat.n, R))
+    M = 80
+    launches0 = h.launch_count
+    mu = host(B.moments(h, dev(L), dev(phi), M))
+    for r in range(R):
+        want = kgo.moments(olat, 0.0, s, L[:, r], phi[:, r], M)
+        assert relerr(mu[r], want) <= TOL
+    # the staged kernel and the one-thread-per-element kernel compute the same steps
+    h.set_option(B.KG_OPT_STAGED, 0)
+    mu_plain = host(B.moments(h, dev(L), dev(phi), M))
+    assert relerr(mu, mu_plain) <= 1e-12
+    assert h.launch_count - launches0 == 2 * M       # (M-1 steps + 1 reduction) twice
+
+
+@pytest.mark.parametrize("alternate", [0, 1])
+@pytest.mark.parametrize("dict_on", [0, 1])
+def test_staged_ring_wraps_many_tiles_per_cta(B, kgo, alternate, dict_on):
+    """62 500 sites x R = 8 = 977 tiles of 512 elements on <= 296 CTAs: every CTA runs several
+    tiles and the 2-3 stage ring wraps; vectors 0 and 7 against the oracle."""
+    lat = sheet(125, 125, 0, True)
+    s = scale_for(lat)
+    olat = to_oracle_lattice(kgo, lat)
+    h = B.from_lattice(lat, lat.x, lat.period_x, 0.0, s)
+    h.set_option(B.KG_OPT_ALTERNATE, alternate)
+    if not dict_on:
+        h.set_option(B.KG_OPT_DICT, 0)
+    R, M = 8, 24
+    phi = W.random_phase_vectors(lat.n, R, 5)
+    mu = host(B.dos_moments(h, dev(phi), M))
+    for r in (0, 7):
+        assert relerr(mu[r], kgo.dos_moments(olat, 0.0, s, phi[:, r], M)) <= TOL
+    again = host(B.dos_moments(h, dev(phi), M))
+    assert mu.tobytes() == again.tobytes()           # bitwise reproducible
+
+
+@pytest.mark.parametrize("stages,ctas", [(2, 1), (2, 3), (4, 1), (6, 1)])
+def test_staged_ring_shapes(B, kgo, stages, ctas):
+    lat = sheet(60, 50, 100, True)                    # 11 900 sites
+    s = scale_for(lat)
+    olat = to_oracle_lattice(kgo, lat)
+    h = B.from_lattice(lat, lat.x, lat.period_x, 0.0, s)
+    h.set_option(B.KG_OPT_STAGES, stages)
+    h.set_option(B.KG_OPT_STAGED_CTAS, ctas)
+    phi = W.random_phase_vectors(lat.n, 1, 6)
+    mu = host(B.dos_moments(h, dev(phi), 40))
+    assert relerr(mu[0], kgo.dos_moments(olat, 0.0, s, phi[:, 0], 40)) <= TOL
+
+
+def test_staged_vac_msd(B, kgo):
+    """Drivers on top of the staged kernel (VAC's first two steps read a strided phi_R and fall
+    back to the plain kernel; MSD is staged from step 2 on)."""
+    lat = sheet(20, 16, 30, True)
+    s = scale_for(lat)
+    olat = to_oracle_lattice(kgo, lat)
+    h = B.from_lattice(lat, lat.x, lat.period_x, 0.0, s)
+    R, M, nt, dt = 2, 48, 2, 0.7
+    phi = W.random_phase_vectors(lat.n, R, 8)
+    vac = host(B.vac(h, dev(phi), M, nt, dt))
+    msd = host(B.msd(h, dev(phi), M, nt, dt))
+    for r in range(R):
+        assert relerr(vac[r], kgo.vac(olat, olat.x, olat.period_x, 0.0, s, phi[:, r], M, nt, dt)) <= TOL
+        assert relerr(msd[r], kgo.msd(olat, olat.x, olat.period_x, 0.0, s, phi[:, r], M, nt, dt)) <= TOL
