@@ -290,7 +290,8 @@ def run_b200(args, cfg):
     bytes_launch = mom_bytes_per_update(R, lat.kmax) * n * R
     achieved = bytes_launch / (kern_us * 1e-6) / 1e9
     traffic = ncu_traffic(f"{cfg.name}_mom_R{R}")
-    roofline = {"bound": "hbm", "kernel": f"kg_step_kernel<R={R}, MODE_MOM> (fused T_m+1 = 2H~T_m - T_m-1 + <phi_L|T_m+1>)",
+    roofline = {"bound": "hbm", "kernel": f"kg_mom_staged_kernel<R={R}> (fused T_m+1 = 2H~T_m - T_m-1 + <phi_L|T_m+1>; "
+                                         "TMA-staged streams, hopping dictionary, alternating sweep)",
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0,
                 "algorithmic_bytes_per_launch": bytes_launch, "us_per_launch": kern_us,
