@@ -178,53 +178,64 @@ static StepArgs base_args(const kg_hamiltonian *h)
     return a;
 }
 
-// ---- staged kernel (kg_staged.cuh): plan + dispatch ----
+// ---- staged kernels (kg_staged.cuh): plan + dispatch ----
 struct StagedPlan { bool ok; int grid, nst, ntiles; size_t smem; };
 
-template <int R, bool ONS, bool DICT>
+template <int R, int MODE, bool ONS, bool DICT>
 static cudaError_t staged_launch_t(const kg_hamiltonian *h, const StagedArgs &a, const StagedPlan &p, cudaStream_t st)
 {
     static size_t configured[64] = {0};
     const int dev = h->device & 63;
     if (configured[dev] < p.smem) {
-        cudaError_t e = cudaFuncSetAttribute(kg_mom_staged_kernel<R, ONS, DICT>,
+        cudaError_t e = cudaFuncSetAttribute(kg_staged_kernel<R, MODE, ONS, DICT>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem);
         if (e != cudaSuccess) return e;
         configured[dev] = p.smem;
     }
-    kg_mom_staged_kernel<R, ONS, DICT><<<p.grid, SG_THREADS, p.smem, st>>>(a);
+    kg_staged_kernel<R, MODE, ONS, DICT><<<p.grid, SG_THREADS, p.smem, st>>>(a);
     return cudaGetLastError();
 }
 
-template <int R>
-static cudaError_t staged_launch_r(const kg_hamiltonian *h, const StagedArgs &a, const StagedPlan &p, cudaStream_t st)
+template <int R, int MODE>
+static cudaError_t staged_launch_rm(const kg_hamiltonian *h, const StagedArgs &a, const StagedPlan &p, cudaStream_t st)
 {
     const bool dict = h->ndict > 0;
-    if (h->has_onsite) return dict ? staged_launch_t<R, true, true>(h, a, p, st) : staged_launch_t<R, true, false>(h, a, p, st);
-    return dict ? staged_launch_t<R, false, true>(h, a, p, st) : staged_launch_t<R, false, false>(h, a, p, st);
+    if (h->has_onsite) return dict ? staged_launch_t<R, MODE, true, true>(h, a, p, st) : staged_launch_t<R, MODE, true, false>(h, a, p, st);
+    return dict ? staged_launch_t<R, MODE, false, true>(h, a, p, st) : staged_launch_t<R, MODE, false, false>(h, a, p, st);
 }
 
-static cudaError_t staged_launch(kg_hamiltonian *h, int R, const StagedArgs &a, const StagedPlan &p, cudaStream_t st)
+template <int MODE>
+static cudaError_t staged_launch_m(const kg_hamiltonian *h, int R, const StagedArgs &a, const StagedPlan &p, cudaStream_t st)
 {
-    h->launches++;
     switch (R) {
-    case 1: return staged_launch_r<1>(h, a, p, st);
-    case 2: return staged_launch_r<2>(h, a, p, st);
-    case 4: return staged_launch_r<4>(h, a, p, st);
-    case 8: return staged_launch_r<8>(h, a, p, st);
+    case 1: return staged_launch_rm<1, MODE>(h, a, p, st);
+    case 2: return staged_launch_rm<2, MODE>(h, a, p, st);
+    case 4: return staged_launch_rm<4, MODE>(h, a, p, st);
+    case 8: return staged_launch_rm<8, MODE>(h, a, p, st);
+    case 16: if (MODE == MODE_EVO) return staged_launch_rm<16, MODE_EVO>(h, a, p, st);
     }
     return cudaErrorInvalidValue;
 }
 
-static StagedPlan staged_plan(const kg_hamiltonian *h, int R)
+static cudaError_t staged_launch(kg_hamiltonian *h, int mode, int R, const StagedArgs &a, const StagedPlan &p, cudaStream_t st)
+{
+    h->launches++;
+    switch (mode) {
+    case MODE_MOM: return staged_launch_m<MODE_MOM>(h, R, a, p, st);
+    case MODE_EVO: return staged_launch_m<MODE_EVO>(h, R, a, p, st);
+    case MODE_PAIR: return staged_launch_m<MODE_PAIR>(h, R, a, p, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+static StagedPlan staged_plan(const kg_hamiltonian *h, int mode, int R)
 {
     StagedPlan p;
     memset(&p, 0, sizeof(p));
-    if (!h->staged || h->kmax != 3 || R > 8) return p;
-    const int cs = SG_TILE_E / R;
-    const size_t stage = ((size_t)SG_TILE_E * 48 + (size_t)cs * 12 + (h->has_onsite ? (size_t)cs * 8 : 0) +
-                          (h->ndict > 0 ? 0 : (size_t)cs * 24) + 127) / 128 * 128;
-    const size_t header = ((size_t)2 * SG_MAX_STAGES * 8 + 128 + (size_t)32 * R * 16 + 127) / 128 * 128;
+    if (!h->staged || h->kmax != 3 || R > (mode == MODE_EVO ? 16 : 8)) return p;
+    const int te = sg_tile_e(mode);
+    const size_t stage = (size_t)sg_stage_bytes(R, mode, h->has_onsite, h->ndict > 0);
+    const size_t header = (size_t)sg_header_bytes(R);
     // auto: 3 CTAs per SM with a 2-deep ring measured best on config 4 (profiles/); fewer CTAs
     // when a stage is too large for that (fp64 hoppings staged)
     int ctas = h->staged_ctas > 0 ? h->staged_ctas : 3, nst = 0;
@@ -237,12 +248,22 @@ static StagedPlan staged_plan(const kg_hamiltonian *h, int R)
     if (nst < 2 || header + (size_t)nst * stage > (size_t)227 * 1024) return p;
     p.nst = nst;
     p.smem = header + (size_t)nst * stage;
-    const int64_t nt = (h->n * R + SG_TILE_E - 1) / SG_TILE_E;
+    const int64_t nt = (h->n * R + te - 1) / te;
     p.ntiles = (int)nt;
     const int64_t cap = (int64_t)h->num_sms * ctas;
     p.grid = (int)(nt < cap ? nt : cap);
     p.ok = true;
     return p;
+}
+
+static StagedArgs staged_base_args(const kg_hamiltonian *h, const StagedPlan &sp)
+{
+    StagedArgs sa;
+    memset(&sa, 0, sizeof(sa));
+    sa.idx = h->ndict > 0 ? h->nlp : h->nl; sa.hop = h->hop; sa.xhop = h->xhop; sa.onsite = h->onsite;
+    memcpy(sa.dict, h->dict, sizeof(sa.dict));
+    sa.n = h->n; sa.ns = h->ns; sa.ntiles = sp.ntiles; sa.nstages = sp.nst;
+    return sa;
 }
 
 static bool r_ok(int R, bool allow16) { return R == 1 || R == 2 || R == 4 || R == 8 || (allow16 && R == 16); }
@@ -569,13 +590,8 @@ static int enqueue_moment_steps(kg_hamiltonian *h, const c128 *phiL, int ldL, co
                                 const StagedPlan &sp, cudaStream_t st)
 {
     const size_t prow = (size_t)grid * R;
-    StagedArgs sa;
-    memset(&sa, 0, sizeof(sa));
-    if (sp.ok) {
-        sa.idx = h->ndict > 0 ? h->nlp : h->nl; sa.hop = h->hop; sa.onsite = h->onsite;
-        memcpy(sa.dict, h->dict, sizeof(sa.dict));
-        sa.n = h->n; sa.ns = h->ns; sa.phiL = phiL; sa.ntiles = sp.ntiles; sa.nstages = sp.nst;
-    }
+    StagedArgs sa = staged_base_args(h, sp);
+    sa.aux = phiL;
     StepArgs a = base_args(h);
     a.phiL = phiL; a.ld_L = ldL;
     // m = 1: T_1 = H~ T_0, partial rows 0 and 1
@@ -593,7 +609,7 @@ static int enqueue_moment_steps(kg_hamiltonian *h, const c128 *phiL, int ldL, co
             // tuned form of the same step: TMA-staged streams, alternating sweep direction
             sa.cur = a.cur; sa.prev = a.prev; sa.next = a.next; sa.partial = a.partial;
             sa.reverse = h->alternate ? (m & 1) : 0;
-            CUDA_TRY(staged_launch(h, R, sa, sp, st));
+            CUDA_TRY(staged_launch(h, MODE_MOM, R, sa, sp, st));
         } else {
             CUDA_TRY(launch_step(h, MODE_MOM, false, R, a, grid, st));
         }
@@ -614,7 +630,7 @@ static int moments_device(kg_hamiltonian *h, const c128 *phiL, int ldL, const c1
                           int M, c128 *mu, int64_t mu_rstride, cudaStream_t st)
 {
     const int64_t elems = h->n * R;
-    const StagedPlan sp = staged_plan(h, R);
+    const StagedPlan sp = staged_plan(h, MODE_MOM, R);
     const int grid = sp.ok ? sp.grid : grid_for(h, elems);   // one partial row shape for both kernels
     void *ta, *tb, *part;
     int rc;
@@ -661,6 +677,9 @@ static int evolve_device(kg_hamiltonian *h, const c128 *in, int ld_in, c128 *out
 {
     const int64_t elems = h->n * R;
     const int grid = grid_for(h, elems);
+    const StagedPlan sp = staged_plan(h, MODE_EVO, R);
+    StagedArgs sa = staged_base_args(h, sp);
+    sa.aux = out; sa.out = out;
     void *ta, *tb;
     int rc;
     if ((rc = ws_get(h, WS_TA, (size_t)elems * 16, &ta)) || (rc = ws_get(h, WS_TB, (size_t)elems * 16, &tb))) return rc;
@@ -679,7 +698,13 @@ static int evolve_device(kg_hamiltonian *h, const c128 *in, int ld_in, c128 *out
         if (m == 2) { a.cur = (c128 *)ta; a.ld_cur = R; a.prev = in; a.ld_prev = ld_in; a.next = (c128 *)tb; }
         else if (m & 1) { a.cur = (c128 *)tb; a.prev = (c128 *)ta; a.ld_prev = R; a.next = (c128 *)ta; }
         else { a.cur = (c128 *)ta; a.prev = (c128 *)tb; a.ld_prev = R; a.next = (c128 *)tb; }
-        CUDA_TRY(launch_step(h, MODE_EVO, false, R, a, grid, st));
+        if (sp.ok && a.ld_cur == R && a.ld_prev == R) {
+            sa.cur = a.cur; sa.prev = a.prev; sa.next = a.next; sa.c1 = a.c1;
+            sa.reverse = h->alternate ? (m & 1) : 0;
+            CUDA_TRY(staged_launch(h, MODE_EVO, R, sa, sp, st));
+        } else {
+            CUDA_TRY(launch_step(h, MODE_EVO, false, R, a, grid, st));
+        }
     }
     return KG_OK;
 }
@@ -698,6 +723,9 @@ static int pair_device(kg_hamiltonian *h, const c128 *psi, const c128 *psix, c12
     std::vector<c128> c;
     series_coefficients(h, dt_fs, eps, c);
     const int np = (int)c.size();
+    const StagedPlan sp = staged_plan(h, MODE_PAIR, R);
+    StagedArgs sa = staged_base_args(h, sp);
+    sa.aux = psi_out; sa.out = psi_out; sa.daux = psix_out; sa.outd = psix_out;
     StepArgs a = base_args(h);
     a.out = psi_out; a.outd = psix_out;
     a.alpha = 1.0;
@@ -719,7 +747,14 @@ static int pair_device(kg_hamiltonian *h, const c128 *psi, const c128 *psix, c12
             a.cur = (c128 *)ta; a.prev = (c128 *)tb; a.next = (c128 *)tb;
             a.dcur = (c128 *)da; a.dprev = (c128 *)db; a.dnext = (c128 *)db;
         }
-        CUDA_TRY(launch_step(h, MODE_PAIR, false, R, a, grid, st));
+        if (sp.ok) {
+            sa.cur = a.cur; sa.prev = a.prev; sa.next = a.next; sa.c1 = a.c1;
+            sa.dcur = a.dcur; sa.dprev = a.dprev; sa.dnext = a.dnext;
+            sa.reverse = h->alternate ? (m & 1) : 0;
+            CUDA_TRY(staged_launch(h, MODE_PAIR, R, sa, sp, st));
+        } else {
+            CUDA_TRY(launch_step(h, MODE_PAIR, false, R, a, grid, st));
+        }
     }
     return KG_OK;
 }

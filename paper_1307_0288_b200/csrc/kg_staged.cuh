@@ -1,9 +1,11 @@
-// kg_staged.cuh — the bandwidth-tuned form of the hot kernel (sm_100a): the fused Chebyshev
-// step  T_{m+1} = 2 H~ T_m - T_{m-1}  (eq 38; Alg. 5 l.6 P:363) with the moment inner
-// product <phi_L|T_{m+1}> (Alg. 5 l.7 P:365, eq 46) folded into the same pass.
+// kg_staged.cuh — the bandwidth-tuned form of the hot kernels (sm_100a): the fused Chebyshev
+// step  T_{m+1} = 2 H~ T_m - T_{m-1}  (eq 38; Alg. 5 l.6 P:363) with, folded into the
+// same pass, the moment inner product <phi_L|T_{m+1}> (Alg. 5 l.7 P:365, eq 46), or the
+// series accumulation out += c_{m+1} T_{m+1} (Alg. 6 l.6 P:385, eq 36), or the commutator
+// recursion of eq 39 (Alg. 7) on the (a, d) pair with both accumulations (eq 44).
 //
-// Same arithmetic as kg_step_kernel<MODE_MOM> (kg_kernels.cuh); what differs is how the bytes
-// move:
+// Same arithmetic as kg_step_kernel<MODE_MOM / MODE_EVO / MODE_PAIR> (kg_kernels.cuh), steps
+// m >= 2 with contiguous vectors; what differs is how the bytes move:
 //
 //  * every CONTIGUOUS stream of a tile — the tile's own T_m, T_{m-1} and phi_L elements, its
 //    neighbour indices and its on-site energies — is fetched by the TMA engine with 1-D bulk
@@ -31,24 +33,28 @@
 #pragma once
 #include "kg_kernels.cuh"
 
-#define SG_TILE_E 512          // elements (site, vector) per tile
+#define SG_TILE_E 512          // largest tile, elements (site, vector); row stride ns is a multiple
 #define SG_CONSUMERS 256       // consumer threads; + one producer warp
 #define SG_THREADS (SG_CONSUMERS + 32)
-#define SG_EPT (SG_TILE_E / SG_CONSUMERS)
 #define SG_IDX_MASK 0x0FFFFFFF // DICT: neighbour index in bits 0..27, dictionary id in 28..31
 #define SG_MAX_STAGES 8
 
 struct StagedArgs {
     const int32_t *idx;    // [3][ns]  DICT: (id << 28) | NL_ik ; else NL_ik
     const double *hop;     // [3][ns]  H_ik / s              (used when !DICT)
+    const double *xhop;    // [3][ns]  (X_i - X_m) H_ik / s  (MODE_PAIR)
     const double *onsite;  // [ns]     (H_ii - E0)/s         (used when ONS)
     double dict[16];       // DICT: hopping value per id, dict[0] = 0
     int64_t n, ns;
     const c128 *cur;       // T_m      [n][R]
     const c128 *prev;      // T_{m-1}  [n][R]
     c128 *next;            // T_{m+1}  [n][R]; may alias prev
-    const c128 *phiL;      // [n][R]
-    c128 *partial;         // [grid][R]
+    const c128 *aux;       // MODE_MOM: phi_L ; MODE_EVO / MODE_PAIR: the accumulator `out` (read side)
+    c128 *partial;         // MODE_MOM: [grid][R]
+    c128 *out;             // MODE_EVO / MODE_PAIR: out += c1 T_{m+1}
+    c128 c1;
+    const c128 *dcur, *dprev, *daux;   // MODE_PAIR d-chain (daux = outd, read side)
+    c128 *dnext, *outd;
     int ntiles;
     int reverse;           // sweep the tiles from the last to the first
     int nstages;
@@ -94,28 +100,50 @@ __device__ __forceinline__ void sg_bulk_g2s(uint32_t dst, const void *src, uint3
                  : "memory");
 }
 
-// byte offsets inside one stage
-template <int R, bool ONS, bool DICT>
+// Tile size per mode: the pair recursion stages six vector streams, so its tile is half as long
+// to keep >= 2 stages x 3 CTAs per SM in shared memory.
+__host__ __device__ constexpr int sg_tile_e(int mode) { return mode == MODE_PAIR ? 256 : 512; }
+__host__ __device__ constexpr int sg_nvec(int mode) { return mode == MODE_PAIR ? 6 : 3; }
+// bytes of one stage / of the header (host planning and device layout use the same formulas)
+__host__ __device__ constexpr int sg_stage_bytes(int R, int mode, bool ons, bool dict)
+{
+    return (sg_nvec(mode) * sg_tile_e(mode) * 16 + (sg_tile_e(mode) / R) * (12 + (ons ? 8 : 0) +
+            (mode == MODE_PAIR ? 24 : 0) + (dict ? 0 : 24)) + 127) / 128 * 128;
+}
+__host__ __device__ constexpr int sg_header_bytes(int R)
+{
+    return (2 * SG_MAX_STAGES * 8 + 16 * 8 + 32 * R * 16 + 127) / 128 * 128;
+}
+
+// byte offsets inside one stage.  Vector slots: 0 self (T_m of the tile), 1 prev (T_{m-1}),
+// 2 aux (phi_L for moments, the series accumulator for evolve / pair), 3-5 the same for the
+// d-chain of the pair recursion.
+template <int R, int MODE, bool ONS, bool DICT>
 struct SgLayout {
-    static constexpr int CS = SG_TILE_E / R;                 // sites per tile
-    static constexpr int OFF_SELF = 0;
-    static constexpr int OFF_PREV = OFF_SELF + SG_TILE_E * 16;
-    static constexpr int OFF_PHIL = OFF_PREV + SG_TILE_E * 16;
-    static constexpr int OFF_IDX = OFF_PHIL + SG_TILE_E * 16;
+    static constexpr int TE = sg_tile_e(MODE);
+    static constexpr int CS = TE / R;                        // sites per tile
+    static constexpr int VEC = TE * 16;
+    static constexpr int OFF_IDX = sg_nvec(MODE) * VEC;
     static constexpr int OFF_ONS = OFF_IDX + 3 * CS * 4;
-    static constexpr int OFF_HOP = OFF_ONS + (ONS ? CS * 8 : 0);
-    static constexpr int STAGE = (OFF_HOP + (DICT ? 0 : 3 * CS * 8) + 127) / 128 * 128;
-    // header: full[8], empty[8] mbarriers, dict[16], reduction scratch [32][R] c128
+    static constexpr int OFF_XHOP = OFF_ONS + (ONS ? CS * 8 : 0);
+    static constexpr int OFF_HOP = OFF_XHOP + (MODE == MODE_PAIR ? 3 * CS * 8 : 0);
+    static constexpr int STAGE = sg_stage_bytes(R, MODE, ONS, DICT);
     static constexpr int OFF_DICT = 2 * SG_MAX_STAGES * 8;
     static constexpr int OFF_RED = OFF_DICT + 16 * 8;
-    static constexpr int HEADER = (OFF_RED + 32 * R * 16 + 127) / 128 * 128;
+    static constexpr int HEADER = sg_header_bytes(R);
+    static_assert(OFF_HOP + (DICT ? 0 : 3 * CS * 8) <= STAGE, "stage layout");
 };
 
-template <int R, bool ONS, bool DICT>
-__global__ void __launch_bounds__(SG_THREADS) kg_mom_staged_kernel(const StagedArgs a)
+// MODE_MOM   next = 2 H~ cur - prev ; partial += <phiL|next>            (Alg. 5 l.6-7)
+// MODE_EVO   next = 2 H~ cur - prev ; out += c1 next                     (Alg. 6 l.5-6)
+// MODE_PAIR  the same on the a-chain, and on the d-chain
+//            dnext = 2([X,H~] cur + H~ dcur) - dprev ; outd += c1 dnext  (eq 39, Alg. 7 l.7-8)
+template <int R, int MODE, bool ONS, bool DICT>
+__global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs a)
 {
-    typedef SgLayout<R, ONS, DICT> L;
-    constexpr int CS = L::CS;
+    typedef SgLayout<R, MODE, ONS, DICT> L;
+    constexpr int CS = L::CS, TE = L::TE, EPT = TE / SG_CONSUMERS;
+    constexpr bool PAIR = MODE == MODE_PAIR;
     extern __shared__ __align__(128) unsigned char sg_smem[];
     uint64_t *bars = reinterpret_cast<uint64_t *>(sg_smem);
     double *dict_s = reinterpret_cast<double *>(sg_smem + L::OFF_DICT);
@@ -149,21 +177,32 @@ __global__ void __launch_bounds__(SG_THREADS) kg_mom_staged_kernel(const StagedA
                 if (a.reverse) t = a.ntiles - 1 - t;
                 const int64_t site0 = (int64_t)t * CS, e0 = site0 * R;
                 const int64_t rem = total - e0;
-                const uint32_t vbytes = (uint32_t)(rem < SG_TILE_E ? rem : SG_TILE_E) * 16u;
+                const uint32_t vbytes = (uint32_t)(rem < TE ? rem : TE) * 16u;
                 const uint32_t full = full0 + 8 * s;
                 sg_mbar_wait(empty0 + 8 * s, ph ^ 1u);
                 const uint32_t sb = sg_smem_u32(stages + (size_t)s * L::STAGE);
-                uint32_t tx = 3u * vbytes + 3u * CS * 4u;
+                uint32_t tx = (uint32_t)sg_nvec(MODE) * vbytes + 3u * CS * 4u;
                 if (ONS) tx += CS * 8u;
+                if (PAIR) tx += 3u * CS * 8u;
                 if (!DICT) tx += 3u * CS * 8u;
                 sg_mbar_expect_tx(full, tx);
-                sg_bulk_g2s(sb + L::OFF_SELF, a.cur + e0, vbytes, full);
-                sg_bulk_g2s(sb + L::OFF_PREV, a.prev + e0, vbytes, full);
-                sg_bulk_g2s(sb + L::OFF_PHIL, a.phiL + e0, vbytes, full);
+                sg_bulk_g2s(sb + 0 * L::VEC, a.cur + e0, vbytes, full);
+                sg_bulk_g2s(sb + 1 * L::VEC, a.prev + e0, vbytes, full);
+                sg_bulk_g2s(sb + 2 * L::VEC, a.aux + e0, vbytes, full);
+                if (PAIR) {
+                    sg_bulk_g2s(sb + 3 * L::VEC, a.dcur + e0, vbytes, full);
+                    sg_bulk_g2s(sb + 4 * L::VEC, a.dprev + e0, vbytes, full);
+                    sg_bulk_g2s(sb + 5 * L::VEC, a.daux + e0, vbytes, full);
+                }
 #pragma unroll
                 for (int k = 0; k < 3; ++k)
                     sg_bulk_g2s(sb + L::OFF_IDX + k * CS * 4, a.idx + k * a.ns + site0, CS * 4u, full);
                 if (ONS) sg_bulk_g2s(sb + L::OFF_ONS, a.onsite + site0, CS * 8u, full);
+                if (PAIR) {
+#pragma unroll
+                    for (int k = 0; k < 3; ++k)
+                        sg_bulk_g2s(sb + L::OFF_XHOP + k * CS * 8, a.xhop + k * a.ns + site0, CS * 8u, full);
+                }
                 if (!DICT) {
 #pragma unroll
                     for (int k = 0; k < 3; ++k)
@@ -181,20 +220,24 @@ __global__ void __launch_bounds__(SG_THREADS) kg_mom_staged_kernel(const StagedA
             if (a.reverse) t = a.ntiles - 1 - t;
             const int64_t site0 = (int64_t)t * CS, e0 = site0 * R;
             const int64_t rem = total - e0;
-            const int ne = (int)(rem < SG_TILE_E ? rem : SG_TILE_E);
+            const int ne = (int)(rem < TE ? rem : TE);
             const unsigned char *sb = stages + (size_t)s * L::STAGE;
-            const c128 *self_s = reinterpret_cast<const c128 *>(sb + L::OFF_SELF);
-            const c128 *prev_s = reinterpret_cast<const c128 *>(sb + L::OFF_PREV);
-            const c128 *phil_s = reinterpret_cast<const c128 *>(sb + L::OFF_PHIL);
+            const c128 *self_s = reinterpret_cast<const c128 *>(sb + 0 * L::VEC);
+            const c128 *prev_s = reinterpret_cast<const c128 *>(sb + 1 * L::VEC);
+            const c128 *aux_s = reinterpret_cast<const c128 *>(sb + 2 * L::VEC);
+            const c128 *dself_s = reinterpret_cast<const c128 *>(sb + 3 * L::VEC);
+            const c128 *dprev_s = reinterpret_cast<const c128 *>(sb + 4 * L::VEC);
+            const c128 *daux_s = reinterpret_cast<const c128 *>(sb + 5 * L::VEC);
             const int32_t *idx_s = reinterpret_cast<const int32_t *>(sb + L::OFF_IDX);
             const double *ons_s = reinterpret_cast<const double *>(sb + L::OFF_ONS);
+            const double *xhop_s = reinterpret_cast<const double *>(sb + L::OFF_XHOP);
             const double *hop_s = reinterpret_cast<const double *>(sb + L::OFF_HOP);
             sg_mbar_wait(full0 + 8 * s, ph);
 
-            c128 v[SG_EPT][3];
-            double hk[SG_EPT][3];
+            c128 v[EPT][3], dv[PAIR ? EPT : 1][3];
+            double hk[EPT][3];
 #pragma unroll
-            for (int q = 0; q < SG_EPT; ++q) {
+            for (int q = 0; q < EPT; ++q) {
                 const int le = tid + q * SG_CONSUMERS;
                 const int ls = le / R;
 #pragma unroll
@@ -209,38 +252,67 @@ __global__ void __launch_bounds__(SG_THREADS) kg_mom_staged_kernel(const StagedA
                         hk[q][k] = hop_s[k * CS + ls];
                     }
                     const int64_t d = m - site0;
-                    if ((uint64_t)d < (uint64_t)CS) v[q][k] = self_s[(int)d * R + r];
-                    else v[q][k] = ld_nc(a.cur + m * R + r);
+                    if ((uint64_t)d < (uint64_t)CS) {
+                        v[q][k] = self_s[(int)d * R + r];
+                        if (PAIR) dv[q][k] = dself_s[(int)d * R + r];
+                    } else {
+                        v[q][k] = ld_nc(a.cur + m * R + r);
+                        if (PAIR) dv[q][k] = ld_nc(a.dcur + m * R + r);
+                    }
                 }
             }
 #pragma unroll
-            for (int q = 0; q < SG_EPT; ++q) {
+            for (int q = 0; q < EPT; ++q) {
                 const int le = tid + q * SG_CONSUMERS;
                 const int ls = le / R;
-                c128 acc = make_double2(0.0, 0.0);
+                c128 acc = make_double2(0.0, 0.0), dacc = make_double2(0.0, 0.0);
                 if (ONS) {
                     const double eps = ons_s[ls];
                     const c128 self = self_s[le];
                     acc.x = eps * self.x; acc.y = eps * self.y;
+                    if (PAIR) {
+                        const c128 dself = dself_s[le];
+                        dacc.x = eps * dself.x; dacc.y = eps * dself.y;
+                    }
                 }
 #pragma unroll
-                for (int k = 0; k < 3; ++k) cfma_r(acc, hk[q][k], v[q][k]);
+                for (int k = 0; k < 3; ++k) {
+                    cfma_r(acc, hk[q][k], v[q][k]);
+                    if (PAIR) {
+                        cfma_r(dacc, xhop_s[k * CS + ls], v[q][k]);     // [X,H~] a_m
+                        cfma_r(dacc, hk[q][k], dv[q][k]);               // H~ d_m
+                    }
+                }
                 if (le < ne) {
                     const c128 p = prev_s[le];
                     const c128 tt = make_double2(fma(2.0, acc.x, -p.x), fma(2.0, acc.y, -p.y));
                     a.next[e0 + le] = tt;
-                    const c128 Lv = phil_s[le];
-                    sum.x = fma(Lv.x, tt.x, fma(Lv.y, tt.y, sum.x));      // conj(L) * t
-                    sum.y = fma(Lv.x, tt.y, fma(-Lv.y, tt.x, sum.y));
+                    if (MODE == MODE_MOM) {
+                        const c128 Lv = aux_s[le];
+                        sum.x = fma(Lv.x, tt.x, fma(Lv.y, tt.y, sum.x));      // conj(L) * t
+                        sum.y = fma(Lv.x, tt.y, fma(-Lv.y, tt.x, sum.y));
+                    } else {
+                        const c128 o = aux_s[le], ct = cmul(a.c1, tt);
+                        a.out[e0 + le] = make_double2(o.x + ct.x, o.y + ct.y);
+                    }
+                    if (PAIR) {
+                        const c128 dp = dprev_s[le];
+                        const c128 dt = make_double2(fma(2.0, dacc.x, -dp.x), fma(2.0, dacc.y, -dp.y));
+                        a.dnext[e0 + le] = dt;
+                        const c128 o = daux_s[le], ct = cmul(a.c1, dt);
+                        a.outd[e0 + le] = make_double2(o.x + ct.x, o.y + ct.y);
+                    }
                 }
             }
             __syncwarp();
             if ((tid & 31) == 0) sg_mbar_arrive(empty0 + 8 * s);
         }
     }
-    // block total per vector r (the producer warp adds zeros)
-    c128 tot = block_reduce_per_r<R>(sum, red);
-    if (tid < R) a.partial[(int64_t)blockIdx.x * R + tid] = tot;
+    if (MODE == MODE_MOM) {
+        // block total per vector r (the producer warp adds zeros)
+        c128 tot = block_reduce_per_r<R>(sum, red);
+        if (tid < R) a.partial[(int64_t)blockIdx.x * R + tid] = tot;
+    }
 }
 
 // ---------------------------------------------------------------------------------------

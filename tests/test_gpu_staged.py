@@ -134,3 +134,54 @@ def test_staged_vac_msd(B, kgo):
     for r in range(R):
         assert relerr(vac[r], kgo.vac(olat, olat.x, olat.period_x, 0.0, s, phi[:, r], M, nt, dt)) <= TOL
         assert relerr(msd[r], kgo.msd(olat, olat.x, olat.period_x, 0.0, s, phi[:, r], M, nt, dt)) <= TOL
+
+
+@pytest.mark.parametrize("R", [1, 8, 16])
+@pytest.mark.parametrize("dict_on", [0, 1])
+def test_staged_evolve_many_tiles(B, kgo, R, dict_on):
+    """Alg. 6 on the staged kernel (MODE_EVO): 62 500 sites, every CTA runs several tiles;
+    against the oracle (vector 0) and against the one-thread-per-element kernel (all vectors)."""
+    lat = sheet(125, 125, 0, True)
+    s = scale_for(lat)
+    olat = to_oracle_lattice(kgo, lat)
+    h = B.from_lattice(lat, lat.x, lat.period_x, 0.0, s)
+    if not dict_on:
+        h.set_option(B.KG_OPT_DICT, 0)
+    phi = W.random_phase_vectors(lat.n, R, 5)
+    dt = -1.7
+    out = host(B.evolve(h, dev(phi), dt))
+    assert relerr(out[:, 0], kgo.evolve(olat, 0.0, s, phi[:, 0].copy(), dt)) <= 1e-12
+    assert np.allclose(np.linalg.norm(out, axis=0), 1.0, atol=1e-12)
+    h.set_option(B.KG_OPT_STAGED, 0)
+    plain = host(B.evolve(h, dev(phi), dt))
+    assert relerr(out, plain) <= 1e-13
+
+
+@pytest.mark.parametrize("R", [1, 4, 8])
+@pytest.mark.parametrize("kind", ["uniform", "many"])
+def test_staged_evolve_x_many_tiles(B, kgo, R, kind):
+    """Eq 44 / Alg. 7 on the staged pair kernel (MODE_PAIR), two consecutive steps so that the
+    second one starts from a non-zero psix; vacancies + on-site disorder; vector R-1 vs oracle."""
+    lat = sheet(110, 90, 300, True)          # 39 300 sites
+    if kind != "uniform":
+        lat = set_hoppings(lat, kind)
+    s = scale_for(lat)
+    olat = to_oracle_lattice(kgo, lat)
+    h = B.from_lattice(lat, lat.x, lat.period_x, 0.0, s)
+    phi = W.random_phase_vectors(lat.n, R, 7)
+    dt = 1.3
+    psi, psix = dev(phi), dev(np.zeros_like(phi))
+    for _ in range(2):
+        B.evolve_x(h, psi, psix, dt)
+    want_psi, want_x = phi[:, R - 1].copy(), np.zeros(lat.n, complex)
+    for _ in range(2):                       # eq 44 with the oracle's literal Alg. 6 + Alg. 7
+        want_x = kgo.evolve(olat, 0.0, s, want_x, dt) + \
+            kgo.comm_evolve(olat, olat.x, olat.period_x, 0.0, s, want_psi, dt)
+        want_psi = kgo.evolve(olat, 0.0, s, want_psi, dt)
+    assert relerr(host(psi)[:, R - 1], want_psi) <= 1e-12
+    assert relerr(host(psix)[:, R - 1], want_x) <= 1e-12
+    h.set_option(B.KG_OPT_STAGED, 0)
+    p2, x2 = dev(phi), dev(np.zeros_like(phi))
+    for _ in range(2):
+        B.evolve_x(h, p2, x2, dt)
+    assert relerr(host(psix), host(x2)) <= 1e-13
