@@ -51,7 +51,7 @@ enum {
 
 struct GraphEntry {
     const void *phiL, *phiR;
-    int ldL, ldR, R, M, grid, threads;
+    int ldL, ldR, R, M, grid, threads, dbl;
     cudaGraphExec_t exec;
 };
 
@@ -65,7 +65,7 @@ struct kg_hamiltonian {
     double *hop, *xhop, *onsite;
     double dict[16];          // hopping dictionary, dict[0] = 0
     int ndict;                // entries in use (0: hoppings do not fit a dictionary)
-    int staged, stages, staged_ctas, alternate;   // options of the staged kernel
+    int staged, stages, staged_ctas, alternate, doubling;   // options of the staged kernel
     void *ws[WS_COUNT];
     size_t ws_bytes[WS_COUNT];
     size_t matrix_bytes;
@@ -164,6 +164,7 @@ static cudaError_t launch_step(kg_hamiltonian *h, int mode, bool first, int R, c
     case MODE_EVO: return first ? launch_mf<MODE_EVO, true>(h, R, a, grid, st) : launch_mf<MODE_EVO, false>(h, R, a, grid, st);
     case MODE_PAIR: return first ? launch_mf<MODE_PAIR, true>(h, R, a, grid, st) : launch_mf<MODE_PAIR, false>(h, R, a, grid, st);
     case MODE_VEL: return launch_mf<MODE_VEL, true>(h, R, a, grid, st);
+    case MODE_MOM2: return first ? launch_mf<MODE_MOM2, true>(h, R, a, grid, st) : launch_mf<MODE_MOM2, false>(h, R, a, grid, st);
     }
     return cudaErrorInvalidValue;
 }
@@ -224,6 +225,7 @@ static cudaError_t staged_launch(kg_hamiltonian *h, int mode, int R, const Stage
     case MODE_MOM: return staged_launch_m<MODE_MOM>(h, R, a, p, st);
     case MODE_EVO: return staged_launch_m<MODE_EVO>(h, R, a, p, st);
     case MODE_PAIR: return staged_launch_m<MODE_PAIR>(h, R, a, p, st);
+    case MODE_MOM2: return staged_launch_m<MODE_MOM2>(h, R, a, p, st);
     }
     return cudaErrorInvalidValue;
 }
@@ -352,7 +354,7 @@ static int create_from_device_list(kg_hamiltonian **out, int64_t n, int kmax, co
     h->n = n; h->ns = (n + SG_TILE_E - 1) / SG_TILE_E * SG_TILE_E; h->kmax = kmax;
     h->s = s; h->e0 = e0; h->period = period;
     h->nl = h->nlp = nullptr; h->hop = h->xhop = h->onsite = nullptr;
-    h->ndict = 0; h->staged = 1; h->stages = 0; h->staged_ctas = 0; h->alternate = 1;
+    h->ndict = 0; h->staged = 1; h->stages = 0; h->staged_ctas = 0; h->alternate = 1; h->doubling = 1;
     memset(h->dict, 0, sizeof(h->dict));
     memset(h->ws, 0, sizeof(h->ws));
     memset(h->ws_bytes, 0, sizeof(h->ws_bytes));
@@ -570,6 +572,7 @@ extern "C" int kg_set_option(kg_hamiltonian *h, int option, int64_t value)
         if (value < 0 || value > 8) return fail(KG_EINVAL, "staged CTAs per SM must be in [0, 8]");
         h->staged_ctas = (int)value; break;
     case KG_OPT_ALTERNATE: h->alternate = value != 0; break;
+    case KG_OPT_DOUBLING: h->doubling = value != 0; break;
     case KG_OPT_DICT:
         if (value != 0) return fail(KG_EINVAL, "the dictionary can only be switched off");
         h->ndict = 0; break;
@@ -587,8 +590,12 @@ extern "C" int kg_set_option(kg_hamiltonian *h, int option, int64_t value)
 // enqueue the M-1 fused recursion+dot kernels of Alg. 5 (a2+a3); partials [M][grid][R]
 static int enqueue_moment_steps(kg_hamiltonian *h, const c128 *phiL, int ldL, const c128 *phiR, int ldR,
                                 int R, int M, c128 *ta, c128 *tb, c128 *part, int grid,
-                                const StagedPlan &sp, cudaStream_t st)
+                                const StagedPlan &sp, bool dbl, cudaStream_t st)
 {
+    // dbl (phi_L = phi_R): step m produces T_m and the partials of moments 2m-1 and 2m, so the
+    // loop stops at m = M/2 (2 T_a T_b = T_{a+b} + T_{|a-b|}; kg_reduce_partials finishes it)
+    const int mode = dbl ? MODE_MOM2 : MODE_MOM;
+    const int m_end = dbl ? M / 2 + 1 : M;
     const size_t prow = (size_t)grid * R;
     StagedArgs sa = staged_base_args(h, sp);
     sa.aux = phiL;
@@ -597,21 +604,22 @@ static int enqueue_moment_steps(kg_hamiltonian *h, const c128 *phiL, int ldL, co
     // m = 1: T_1 = H~ T_0, partial rows 0 and 1
     a.alpha = 1.0;
     a.cur = phiR; a.ld_cur = ldR; a.next = ta;
-    a.partial0 = part; a.partial = part + prow;
-    CUDA_TRY(launch_step(h, MODE_MOM, true, R, a, grid, st));
+    a.partial0 = part; a.partial = part + prow; a.partial2 = part + 2 * prow;
+    CUDA_TRY(launch_step(h, mode, true, R, a, grid, st));
     a.alpha = 2.0; a.partial0 = nullptr;
-    for (int m = 2; m < M; ++m) {
-        a.partial = part + (size_t)m * prow;
+    for (int m = 2; m < m_end; ++m) {
+        a.partial = part + (size_t)(dbl ? 2 * m - 1 : m) * prow;
+        a.partial2 = part + (size_t)(2 * m) * prow;
         if (m == 2) { a.cur = ta; a.ld_cur = R; a.prev = phiR; a.ld_prev = ldR; a.next = tb; }
         else if (m & 1) { a.cur = tb; a.ld_cur = R; a.prev = ta; a.ld_prev = R; a.next = ta; }
         else { a.cur = ta; a.ld_cur = R; a.prev = tb; a.ld_prev = R; a.next = tb; }
         if (sp.ok && ldL == R && a.ld_cur == R && a.ld_prev == R) {
             // tuned form of the same step: TMA-staged streams, alternating sweep direction
-            sa.cur = a.cur; sa.prev = a.prev; sa.next = a.next; sa.partial = a.partial;
+            sa.cur = a.cur; sa.prev = a.prev; sa.next = a.next; sa.partial = a.partial; sa.partial2 = a.partial2;
             sa.reverse = h->alternate ? (m & 1) : 0;
-            CUDA_TRY(staged_launch(h, MODE_MOM, R, sa, sp, st));
+            CUDA_TRY(staged_launch(h, mode, R, sa, sp, st));
         } else {
-            CUDA_TRY(launch_step(h, MODE_MOM, false, R, a, grid, st));
+            CUDA_TRY(launch_step(h, mode, false, R, a, grid, st));
         }
     }
     return KG_OK;
@@ -630,24 +638,25 @@ static int moments_device(kg_hamiltonian *h, const c128 *phiL, int ldL, const c1
                           int M, c128 *mu, int64_t mu_rstride, cudaStream_t st)
 {
     const int64_t elems = h->n * R;
-    const StagedPlan sp = staged_plan(h, MODE_MOM, R);
+    const bool dbl = h->doubling && phiL == phiR && ldL == ldR;
+    const StagedPlan sp = staged_plan(h, dbl ? MODE_MOM2 : MODE_MOM, R);
     const int grid = sp.ok ? sp.grid : grid_for(h, elems);   // one partial row shape for both kernels
     void *ta, *tb, *part;
     int rc;
     if ((rc = ws_get(h, WS_TA, (size_t)elems * 16, &ta)) || (rc = ws_get(h, WS_TB, (size_t)elems * 16, &tb)) ||
-        (rc = ws_get(h, WS_PART, (size_t)M * grid * R * 16, &part)))
+        (rc = ws_get(h, WS_PART, (size_t)(M + 1) * grid * R * 16, &part)))
         return rc;
     if (want_graph(h, elems, st)) {
         cudaGraphExec_t exec = nullptr;
         for (auto &g : h->graphs)
             if (g.phiL == phiL && g.phiR == phiR && g.ldL == ldL && g.ldR == ldR && g.R == R && g.M == M &&
-                g.grid == grid && g.threads == h->threads)
+                g.grid == grid && g.threads == h->threads && g.dbl == (int)dbl)
                 exec = g.exec;
         if (!exec) {
             cudaGraph_t graph;
             CUDA_TRY(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
             const int64_t before = h->launches;
-            rc = enqueue_moment_steps(h, phiL, ldL, phiR, ldR, R, M, (c128 *)ta, (c128 *)tb, (c128 *)part, grid, sp, st);
+            rc = enqueue_moment_steps(h, phiL, ldL, phiR, ldR, R, M, (c128 *)ta, (c128 *)tb, (c128 *)part, grid, sp, dbl, st);
             h->launches = before;
             cudaError_t e = cudaStreamEndCapture(st, &graph);
             if (rc) { if (e == cudaSuccess) cudaGraphDestroy(graph); return rc; }
@@ -656,16 +665,16 @@ static int moments_device(kg_hamiltonian *h, const c128 *phiL, int ldL, const c1
             cudaGraphDestroy(graph);
             if (e != cudaSuccess) return fail(KG_ECUDA, "graph instantiate: %s", cudaGetErrorString(e));
             if (h->graphs.size() >= 8) { cudaGraphExecDestroy(h->graphs.front().exec); h->graphs.erase(h->graphs.begin()); }
-            h->graphs.push_back(GraphEntry{phiL, phiR, ldL, ldR, R, M, grid, h->threads, exec});
+            h->graphs.push_back(GraphEntry{phiL, phiR, ldL, ldR, R, M, grid, h->threads, (int)dbl, exec});
         }
         CUDA_TRY(cudaGraphLaunch(exec, st));
-        h->launches += M - 1;
+        h->launches += dbl ? M / 2 : M - 1;
     } else {
-        if ((rc = enqueue_moment_steps(h, phiL, ldL, phiR, ldR, R, M, (c128 *)ta, (c128 *)tb, (c128 *)part, grid, sp, st)))
+        if ((rc = enqueue_moment_steps(h, phiL, ldL, phiR, ldR, R, M, (c128 *)ta, (c128 *)tb, (c128 *)part, grid, sp, dbl, st)))
             return rc;
     }
     const int warps = M * R;
-    kg_reduce_partials<<<(warps * 32 + 255) / 256, 256, 0, st>>>((const c128 *)part, M, grid, R, mu, mu_rstride);
+    kg_reduce_partials<<<(warps * 32 + 255) / 256, 256, 0, st>>>((const c128 *)part, M, grid, R, mu, mu_rstride, dbl ? 1 : 0);
     h->launches++;
     CUDA_TRY(cudaGetLastError());
     return KG_OK;

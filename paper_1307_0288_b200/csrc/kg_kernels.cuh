@@ -4,6 +4,9 @@
 //
 //   MODE_MOM   T_{m+1} = alpha H~ T_m - beta T_{m-1}  (eq 38)  + per-block partial of
 //              <phi_L|T_{m+1}>  (Alg. 5 l.6-7 P:363-365; the paper's K3 and K5 in one pass)
+//   MODE_MOM2  the same recursion for phi_L = phi_R = phi with the product identity
+//              2 T_a T_b = T_{a+b} + T_{|a-b|}: per-block partials of <T_m|T_{m+1}> (moment
+//              2m+1) and <T_{m+1}|T_{m+1}> (moment 2m+2) — two moments per sweep, no phi_L read
 //   MODE_EVO   same recursion + out (+)= c_{m+1} T_{m+1}              (Alg. 6 l.5-6 P:383-385)
 //   MODE_PAIR  (a, d) pair recursion: a = T_m psi, d = T_m psix + [X,T_m] psi,
 //              d_{m+1} = alpha([X,H~] a_m + H~ d_m) - beta d_{m-1}    (eq 39, Alg. 7 l.7-8)
@@ -26,7 +29,7 @@
 
 typedef double2 c128;
 
-enum { MODE_MOM = 0, MODE_EVO = 1, MODE_PAIR = 2, MODE_VEL = 3 };
+enum { MODE_MOM = 0, MODE_EVO = 1, MODE_PAIR = 2, MODE_VEL = 3, MODE_MOM2 = 4 };
 
 struct StepArgs {
     // matrix (device, library-owned)
@@ -46,6 +49,7 @@ struct StepArgs {
     const c128 *phiL; int ld_L;
     c128 *partial;                   // [grid][R] for moment m+1
     c128 *partial0;                  // FIRST only: [grid][R] for moment 0
+    c128 *partial2;                  // MODE_MOM2: [grid][R] for moment 2m+2 (partial: 2m+1)
     // MODE_EVO / MODE_PAIR: series accumulators (ld = R)
     c128 *out;
     c128 c0, c1;                     // FIRST: out = c0 cur + c1 next; else out += c1 next
@@ -107,14 +111,14 @@ __global__ void __launch_bounds__(256) kg_step_kernel(const StepArgs a)
     const int r = threadIdx.x & (R - 1);
     const int kmax = KMAX > 0 ? KMAX : a.kmax;
 
-    c128 sum = make_double2(0.0, 0.0), sum0 = make_double2(0.0, 0.0);
+    c128 sum = make_double2(0.0, 0.0), sum0 = make_double2(0.0, 0.0), sum2 = make_double2(0.0, 0.0);
 
     for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += stride) {
         const int64_t i = e / R;   // R is a power of two: a shift
         c128 acc = make_double2(0.0, 0.0);
         c128 dacc = make_double2(0.0, 0.0);
         c128 self = make_double2(0.0, 0.0), dself = make_double2(0.0, 0.0);
-        if (MODE != MODE_VEL && (ONS || FIRST)) {
+        if (MODE != MODE_VEL && (ONS || FIRST || MODE == MODE_MOM2)) {
             self = ld_nc(a.cur + i * a.ld_cur + r);
             if (MODE == MODE_PAIR) dself = ld_nc(a.dcur + i * a.ld_dcur + r);
         }
@@ -162,6 +166,12 @@ __global__ void __launch_bounds__(256) kg_step_kernel(const StepArgs a)
                 sum0.y = fma(L.x, self.y, fma(-L.y, self.x, sum0.y));
             }
         }
+        if (MODE == MODE_MOM2) {
+            sum.x = fma(self.x, t.x, fma(self.y, t.y, sum.x));        // conj(T_m) * T_{m+1}
+            sum.y = fma(self.x, t.y, fma(-self.y, t.x, sum.y));
+            sum2.x = fma(t.x, t.x, fma(t.y, t.y, sum2.x));            // |T_{m+1}|^2
+            if (FIRST) sum0.x = fma(self.x, self.x, fma(self.y, self.y, sum0.x));
+        }
         if (MODE == MODE_EVO || MODE == MODE_PAIR) {
             c128 o;
             if (FIRST) o = cmul(a.c0, self); else o = a.out[e];
@@ -184,10 +194,14 @@ __global__ void __launch_bounds__(256) kg_step_kernel(const StepArgs a)
         }
     }
 
-    if (MODE == MODE_MOM) {
+    if (MODE == MODE_MOM || MODE == MODE_MOM2) {
         __shared__ c128 red[32 * R];
         c128 tot = block_reduce_per_r<R>(sum, red);
         if (threadIdx.x < R) a.partial[(int64_t)blockIdx.x * R + threadIdx.x] = tot;
+        if (MODE == MODE_MOM2) {
+            c128 tot2 = block_reduce_per_r<R>(sum2, red);
+            if (threadIdx.x < R) a.partial2[(int64_t)blockIdx.x * R + threadIdx.x] = tot2;
+        }
         if (FIRST) {
             c128 tot0 = block_reduce_per_r<R>(sum0, red);
             if (threadIdx.x < R) a.partial0[(int64_t)blockIdx.x * R + threadIdx.x] = tot0;
@@ -197,8 +211,10 @@ __global__ void __launch_bounds__(256) kg_step_kernel(const StepArgs a)
 
 // Fixed-order final sum of the per-block partials (a8): one warp per (moment m, vector r).
 // partials [M][B][R]  ->  mu[r*mu_rstride + m]
+// `doubling`: rows m >= 2 hold <T_a|T_b> with a + b = m, |a - b| = m & 1, and
+// mu_m = 2 <T_a|T_b> - mu_{m&1}  (2 T_a T_b = T_{a+b} + T_{|a-b|}).
 __global__ void kg_reduce_partials(const c128 *__restrict__ partials, int M, int B, int R,
-                                   c128 *__restrict__ mu, int64_t mu_rstride)
+                                   c128 *__restrict__ mu, int64_t mu_rstride, int doubling)
 {
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
@@ -214,6 +230,20 @@ __global__ void kg_reduce_partials(const c128 *__restrict__ partials, int M, int
     for (int off = 16; off >= 1; off >>= 1) {
         sx += __shfl_xor_sync(0xffffffffu, sx, off);
         sy += __shfl_xor_sync(0xffffffffu, sy, off);
+    }
+    if (doubling && m >= 2) {
+        const c128 *p0 = partials + (int64_t)(m & 1) * B * R + r;
+        double bx = 0.0, by = 0.0;
+        for (int b = lane; b < B; b += 32) {
+            const c128 v = p0[(int64_t)b * R];
+            bx += v.x; by += v.y;
+        }
+#pragma unroll
+        for (int off = 16; off >= 1; off >>= 1) {
+            bx += __shfl_xor_sync(0xffffffffu, bx, off);
+            by += __shfl_xor_sync(0xffffffffu, by, off);
+        }
+        sx = 2.0 * sx - bx; sy = 2.0 * sy - by;
     }
     if (lane == 0) mu[(int64_t)r * mu_rstride + m] = make_double2(sx, sy);
 }

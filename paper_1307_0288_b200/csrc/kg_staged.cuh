@@ -50,7 +50,8 @@ struct StagedArgs {
     const c128 *prev;      // T_{m-1}  [n][R]
     c128 *next;            // T_{m+1}  [n][R]; may alias prev
     const c128 *aux;       // MODE_MOM: phi_L ; MODE_EVO / MODE_PAIR: the accumulator `out` (read side)
-    c128 *partial;         // MODE_MOM: [grid][R]
+    c128 *partial;         // MODE_MOM: [grid][R] ; MODE_MOM2: <T_m|T_{m+1}> (moment 2m+1)
+    c128 *partial2;        // MODE_MOM2: <T_{m+1}|T_{m+1}> (moment 2m+2)
     c128 *out;             // MODE_EVO / MODE_PAIR: out += c1 T_{m+1}
     c128 c1;
     const c128 *dcur, *dprev, *daux;   // MODE_PAIR d-chain (daux = outd, read side)
@@ -103,7 +104,7 @@ __device__ __forceinline__ void sg_bulk_g2s(uint32_t dst, const void *src, uint3
 // Tile size per mode: the pair recursion stages six vector streams, so its tile is half as long
 // to keep >= 2 stages x 3 CTAs per SM in shared memory.
 __host__ __device__ constexpr int sg_tile_e(int mode) { return mode == MODE_PAIR ? 256 : 512; }
-__host__ __device__ constexpr int sg_nvec(int mode) { return mode == MODE_PAIR ? 6 : 3; }
+__host__ __device__ constexpr int sg_nvec(int mode) { return mode == MODE_PAIR ? 6 : mode == MODE_MOM2 ? 2 : 3; }
 // bytes of one stage / of the header (host planning and device layout use the same formulas)
 __host__ __device__ constexpr int sg_stage_bytes(int R, int mode, bool ons, bool dict)
 {
@@ -135,6 +136,8 @@ struct SgLayout {
 };
 
 // MODE_MOM   next = 2 H~ cur - prev ; partial += <phiL|next>            (Alg. 5 l.6-7)
+// MODE_MOM2  next = 2 H~ cur - prev ; partial += <cur|next>, partial2 += <next|next>
+//            (phi_L = phi_R: moments 2m+1 and 2m+2 from one sweep, see kg_kernels.cuh)
 // MODE_EVO   next = 2 H~ cur - prev ; out += c1 next                     (Alg. 6 l.5-6)
 // MODE_PAIR  the same on the a-chain, and on the d-chain
 //            dnext = 2([X,H~] cur + H~ dcur) - dprev ; outd += c1 dnext  (eq 39, Alg. 7 l.7-8)
@@ -165,7 +168,7 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
 
     const int64_t total = a.n * R;
     const int my_tiles = ((int)blockIdx.x < a.ntiles) ? (a.ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
-    c128 sum = make_double2(0.0, 0.0);
+    c128 sum = make_double2(0.0, 0.0), sum2 = make_double2(0.0, 0.0);
 
     if (tid >= SG_CONSUMERS) {
         // ---------------- producer warp: one lane feeds the ring ----------------
@@ -188,7 +191,7 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
                 sg_mbar_expect_tx(full, tx);
                 sg_bulk_g2s(sb + 0 * L::VEC, a.cur + e0, vbytes, full);
                 sg_bulk_g2s(sb + 1 * L::VEC, a.prev + e0, vbytes, full);
-                sg_bulk_g2s(sb + 2 * L::VEC, a.aux + e0, vbytes, full);
+                if (MODE != MODE_MOM2) sg_bulk_g2s(sb + 2 * L::VEC, a.aux + e0, vbytes, full);
                 if (PAIR) {
                     sg_bulk_g2s(sb + 3 * L::VEC, a.dcur + e0, vbytes, full);
                     sg_bulk_g2s(sb + 4 * L::VEC, a.dprev + e0, vbytes, full);
@@ -291,6 +294,11 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
                         const c128 Lv = aux_s[le];
                         sum.x = fma(Lv.x, tt.x, fma(Lv.y, tt.y, sum.x));      // conj(L) * t
                         sum.y = fma(Lv.x, tt.y, fma(-Lv.y, tt.x, sum.y));
+                    } else if (MODE == MODE_MOM2) {
+                        const c128 sv = self_s[le];
+                        sum.x = fma(sv.x, tt.x, fma(sv.y, tt.y, sum.x));      // conj(T_m) * T_{m+1}
+                        sum.y = fma(sv.x, tt.y, fma(-sv.y, tt.x, sum.y));
+                        sum2.x = fma(tt.x, tt.x, fma(tt.y, tt.y, sum2.x));    // |T_{m+1}|^2
                     } else {
                         const c128 o = aux_s[le], ct = cmul(a.c1, tt);
                         a.out[e0 + le] = make_double2(o.x + ct.x, o.y + ct.y);
@@ -308,10 +316,14 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
             if ((tid & 31) == 0) sg_mbar_arrive(empty0 + 8 * s);
         }
     }
-    if (MODE == MODE_MOM) {
+    if (MODE == MODE_MOM || MODE == MODE_MOM2) {
         // block total per vector r (the producer warp adds zeros)
         c128 tot = block_reduce_per_r<R>(sum, red);
         if (tid < R) a.partial[(int64_t)blockIdx.x * R + tid] = tot;
+        if (MODE == MODE_MOM2) {
+            c128 tot2 = block_reduce_per_r<R>(sum2, red);
+            if (tid < R) a.partial2[(int64_t)blockIdx.x * R + tid] = tot2;
+        }
     }
 }
 

@@ -185,3 +185,30 @@ def test_staged_evolve_x_many_tiles(B, kgo, R, kind):
     for _ in range(2):
         B.evolve_x(h, p2, x2, dt)
     assert relerr(host(psix), host(x2)) <= 1e-13
+
+
+@pytest.mark.parametrize("M", [2, 3, 4, 63, 64])
+@pytest.mark.parametrize("R", [1, 4])
+@pytest.mark.parametrize("staged", [0, 1])
+def test_doubling_moments(B, kgo, M, R, staged):
+    """phi_L = phi_R: two moments per Chebyshev step from 2 T_a T_b = T_{a+b} + T_{|a-b|}
+    (mu_{2n+1} = 2<T_n|T_{n+1}> - mu_1, mu_{2n+2} = 2<T_{n+1}|T_{n+1}> - mu_0) against the
+    oracle's literal Alg. 5, for odd / even / minimal M, and against the literal GPU path."""
+    lat = sheet(30, 26, 77, True)          # 3043 sites
+    s = scale_for(lat)
+    olat = to_oracle_lattice(kgo, lat)
+    h = B.from_lattice(lat, lat.x, lat.period_x, 0.0, s)
+    h.set_option(B.KG_OPT_STAGED, staged)
+    rng = np.random.default_rng(M)
+    phi = rng.normal(size=(lat.n, R)) + 1j * rng.normal(size=(lat.n, R))     # not normalised
+    d = dev(phi)
+    l0 = h.launch_count
+    mu = host(B.dos_moments(h, d, M))
+    assert h.launch_count - l0 == M // 2 + 1                # M/2 sweeps + the reduction
+    for r in range(R):
+        assert relerr(mu[r], kgo.dos_moments(olat, 0.0, s, phi[:, r].copy(), M)) <= TOL
+    h.set_option(B.KG_OPT_DOUBLING, 0)
+    l0 = h.launch_count
+    lit = host(B.dos_moments(h, d, M))
+    assert h.launch_count - l0 == M                         # literal Alg. 5: M-1 sweeps + reduction
+    assert relerr(mu, lit) <= 1e-13
