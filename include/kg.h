@@ -172,6 +172,23 @@ int kg_msd(kg_hamiltonian *h, const kg_c128 *phi, int R, int M, int n_steps, dou
  */
 int kg_bessel_terms(double x, double bessel_eps, int *np_out, double *j, int cap);
 
+/*
+ * kg_kpm_reconstruct — kernel-polynomial reconstruction of a function of energy from Chebyshev
+ * moments (eqs 29-31) with Jackson damping (eq 35), for unit-norm phi:
+ *   f[row][j] = 1/(pi s sqrt(1 - x_j^2)) * sum_{m<M} g_m (2 - delta_m0) T_m(x_j) Re mu[row][m],
+ *   x_j = (E_j - E0)/s,  g_m = (1 - m a) cos(pi m a) + a sin(pi m a) cot(pi a),  a = 1/(M+1).
+ * Applied to kg_dos_moments it gives rho(E) per site and spin (1/eV, integrates to 1); to a row
+ * of kg_vac / kg_msd it gives rho(E) C_vv(E,t) (nm^2/fs^2/eV) / rho(E) DeltaX^2(E,t) (nm^2/eV).
+ *   mu        [rows][M] complex128 (any leading shape flattened to rows), host or device
+ *   jackson   1: g_m as above; 0: g_m = 1 (Dirichlet)
+ *   energies_eV [n_energies], host or device; every |x_j| must be < 1 (else KG_EINVAL)
+ *   f         [rows][n_energies] fp64, host or device
+ * Runs as CUDA kernels on `stream` and synchronises it before returning.
+ */
+int kg_kpm_reconstruct(const kg_c128 *mu, int64_t rows, int M, int jackson, double e0_eV,
+                       double scale_eV, const double *energies_eV, int n_energies, double *f,
+                       void *stream);
+
 /* Tuning / introspection (not part of the paper's problem statement). */
 enum {
     KG_OPT_USE_GRAPHS = 1,   /* 1 (default): replay the moment loop as a CUDA graph */

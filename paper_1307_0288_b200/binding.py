@@ -49,6 +49,7 @@ _lib.kg_vac.argtypes = [_vp, _vp, _int, _int, _int, _dbl, _dbl, _vp, _vp]
 _lib.kg_msd.argtypes = [_vp, _vp, _int, _int, _int, _dbl, _dbl, _vp, _vp]
 _lib.kg_bessel_terms.argtypes = [_dbl, _dbl, C.POINTER(_int), _vp, _int]
 _lib.kg_set_option.argtypes = [_vp, _int, _i64]
+_lib.kg_kpm_reconstruct.argtypes = [_vp, _i64, _int, _int, _dbl, _dbl, _vp, _int, _vp, _vp]
 
 
 class KgError(RuntimeError):
@@ -220,3 +221,19 @@ def bessel_terms(x, bessel_eps=1e-15):
     j = np.empty(n_p.value)
     _check(_lib.kg_bessel_terms(x, bessel_eps, C.byref(n_p), j.ctypes.data, n_p.value))
     return n_p.value, j
+
+
+def kpm_reconstruct(mu, e0_eV, scale_eV, energies_eV, jackson=True, stream=None):
+    """kg_kpm_reconstruct: mu [..., M] complex128 (torch or numpy, host or device) ->
+    f [..., n_energies] float64 of the same kind (eqs 29-31, 35)."""
+    M = int(mu.shape[-1])
+    lead = tuple(mu.shape[:-1])
+    rows = int(np.prod(lead)) if lead else 1
+    ne = int(energies_eV.shape[0])
+    if isinstance(mu, np.ndarray):
+        f = np.empty(lead + (ne,), np.float64)
+    else:
+        f = torch.empty(lead + (ne,), dtype=torch.float64, device=mu.device)
+    _check(_lib.kg_kpm_reconstruct(_ptr(mu), rows, M, int(bool(jackson)), float(e0_eV), float(scale_eV),
+                                   _ptr(energies_eV), ne, _ptr(f), _stream(stream)))
+    return f

@@ -954,3 +954,42 @@ extern "C" int kg_msd(kg_hamiltonian *h, const kg_c128 *phi, int R, int M, int n
     }
     return finish_out(o, st);
 }
+
+// --------------------------------------------------------------------------------------
+// KPM reconstruction (SUPPORT row R1/R2 of SURVEY 2.2): handle-free, temporary device buffers
+// --------------------------------------------------------------------------------------
+extern "C" int kg_kpm_reconstruct(const kg_c128 *mu, int64_t rows, int M, int jackson, double e0_eV,
+                                  double scale_eV, const double *energies_eV, int n_energies, double *f,
+                                  void *stream)
+{
+    if (!mu || !energies_eV || !f) return fail(KG_EINVAL, "kg_kpm_reconstruct: NULL argument");
+    if (rows <= 0 || rows > 65535 || M < 1 || n_energies < 1)
+        return fail(KG_EINVAL, "kg_kpm_reconstruct: need 1 <= rows <= 65535, M >= 1, n_energies >= 1");
+    if (!(scale_eV > 0.0) || !std::isfinite(scale_eV) || !std::isfinite(e0_eV))
+        return fail(KG_EINVAL, "kg_kpm_reconstruct: scale must be positive and finite");
+    cudaStream_t st = (cudaStream_t)stream;
+    std::vector<double> en((size_t)n_energies);
+    CUDA_TRY(cudaMemcpyAsync(en.data(), energies_eV, (size_t)n_energies * 8, cudaMemcpyDefault, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    for (double e : en)
+        if (!(std::fabs((e - e0_eV) / scale_eV) < 1.0))
+            return fail(KG_EINVAL, "kg_kpm_reconstruct: energy %.6g eV is outside (E0 - s, E0 + s)", e);
+    TmpDev tmp;
+    const void *d_mu, *d_en;
+    int rc;
+    if ((rc = tmp.get(mu, (size_t)rows * M * 16, st, &d_mu)) || (rc = tmp.get(energies_eV, (size_t)n_energies * 8, st, &d_en)))
+        return rc;
+    double *d_w = nullptr, *d_f = nullptr;
+    CUDA_TRY(cudaMalloc(&d_w, (size_t)M * 8)); tmp.ptrs.push_back(d_w);
+    const bool f_dev = is_device_ptr(f);
+    if (f_dev) d_f = f;
+    else { CUDA_TRY(cudaMalloc(&d_f, (size_t)rows * n_energies * 8)); tmp.ptrs.push_back(d_f); }
+    kg_kpm_weights<<<(M + 255) / 256, 256, 0, st>>>(M, jackson, d_w);
+    dim3 grid((n_energies + 127) / 128, (unsigned)rows);
+    kg_kpm_reconstruct_kernel<<<grid, 128, 0, st>>>((const c128 *)d_mu, rows, M, d_w, e0_eV, scale_eV,
+                                                    (const double *)d_en, n_energies, d_f);
+    CUDA_TRY(cudaGetLastError());
+    if (!f_dev) CUDA_TRY(cudaMemcpyAsync(f, d_f, (size_t)rows * n_energies * 8, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));     // temporaries are freed on return
+    return KG_OK;
+}

@@ -359,3 +359,47 @@ __global__ void kg_csr_max_row(int64_t n, const int64_t *__restrict__ rowptr, in
     }
     atomicMax(maxrow, mx);
 }
+
+// ---------------------------------------------------------------------------------------
+// KPM reconstruction (eqs 29-31, Jackson damping eq 35).
+// w[m] = g_m (2 - delta_m0),  g_m = (1 - m a) cos(pi m a) + a sin(pi m a) cot(pi a), a = 1/(M+1)
+// ---------------------------------------------------------------------------------------
+__global__ void kg_kpm_weights(int M, int jackson, double *__restrict__ w)
+{
+    const int m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= M) return;
+    double g = 1.0;
+    if (jackson) {
+        const double a = 1.0 / (M + 1.0);
+        double sn, cs, sa, ca;
+        sincospi(m * a, &sn, &cs);
+        sincospi(a, &sa, &ca);
+        g = (1.0 - m * a) * cs + a * sn * (ca / sa);
+    }
+    w[m] = (m == 0 ? 1.0 : 2.0) * g;
+}
+
+// f[row][j] = 1/(pi s sqrt(1 - x_j^2)) sum_m w[m] T_m(x_j) Re mu[row][m],  x_j = (E_j - E0)/s,
+// T_m by the three-term recurrence; one thread per (row, energy).
+__global__ void kg_kpm_reconstruct_kernel(const c128 *__restrict__ mu, int64_t rows, int M,
+                                          const double *__restrict__ w, double e0, double s,
+                                          const double *__restrict__ energies, int ne,
+                                          double *__restrict__ f)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t row = blockIdx.y;
+    if (j >= ne || row >= rows) return;
+    const double x = (energies[j] - e0) / s;
+    const c128 *mr = mu + row * (int64_t)M;
+    double t0 = 1.0, t1 = x;
+    double sum = w[0] * mr[0].x, comp = 0.0;           // Kahan-compensated
+    for (int m = 1; m < M; ++m) {
+        const double term = w[m] * t1 * mr[m].x - comp;
+        const double ns = sum + term;
+        comp = (ns - sum) - term;
+        sum = ns;
+        const double t2 = fma(2.0 * x, t1, -t0);
+        t0 = t1; t1 = t2;
+    }
+    f[row * (int64_t)ne + j] = sum / (3.14159265358979323846 * s * sqrt(1.0 - x * x));
+}

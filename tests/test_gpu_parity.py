@@ -312,3 +312,31 @@ def test_tiny_and_isolated_sites(B, kgo):
     phi = rand_vectors(lat.n, 1, 5)
     assert relerr(host(B.msd(h, dev(phi), 16, 2, 0.5))[0],
                   kgo.msd(olat, olat.x, olat.period_x, 0.0, s, phi[:, 0], 16, 2, 0.5)) <= TOL
+
+
+# --------------------------------------------------------------------------------- reconstruction
+@pytest.mark.parametrize("jackson", [True, False])
+def test_kpm_reconstruct(B, kgo, jackson):
+    """eqs 29-31 + Jackson kernel (eq 35) on the device against the oracle: config 1's DOS on its
+    1001-point grid (M = 256), MSD rows (several rows at once), host and device pointers."""
+    cfg = W.make_config(1)
+    lat = cfg.lattice
+    h = B.from_lattice(lat, cfg.xcoord, cfg.period, cfg.e0, cfg.scale)
+    phi = dev(W.random_phase_vectors(lat.n, 1, cfg.seed))
+    en = W.energy_grid(cfg.n_energies)
+    mu = B.dos_moments(h, phi, cfg.M)
+    rho = host(B.kpm_reconstruct(mu, cfg.e0, cfg.scale, dev(en), jackson))
+    want = kgo.kpm_reconstruct(host(mu)[0], cfg.e0, cfg.scale, en, jackson)
+    assert rho.shape == (1, cfg.n_energies)
+    assert relerr(rho[0], want) <= TOL
+    if jackson:
+        assert np.all(rho > 0)
+        assert abs(np.sum(0.5 * (rho[0, 1:] + rho[0, :-1]) * np.diff(en)) - 1.0) < 2e-2   # int rho dE = 1
+    msd = host(B.msd(h, phi, 64, 3, cfg.dt_fs))                   # [1][4][64]
+    f = B.kpm_reconstruct(msd, cfg.e0, cfg.scale, en, jackson)     # numpy in -> numpy out
+    assert f.shape == (1, 4, cfg.n_energies)
+    for k in range(4):
+        assert relerr(f[0, k], kgo.kpm_reconstruct(msd[0, k], cfg.e0, cfg.scale, en, jackson)) <= TOL
+    with pytest.raises(B.KgError) as e:
+        B.kpm_reconstruct(mu, cfg.e0, cfg.scale, np.array([0.0, cfg.scale]), jackson)
+    assert e.value.code == B.KG_EINVAL
