@@ -189,6 +189,26 @@ int kg_kpm_reconstruct(const kg_c128 *mu, int64_t rows, int M, int jackson, doub
                        double scale_eV, const double *energies_eV, int n_energies, double *f,
                        void *stream);
 
+/*
+ * kg_transport — running conductivities and ballistic length / conductance on a (t_k, E_j) grid,
+ * t_k = k dt, k = 0..n_steps, from reconstructed functions (kg_kpm_reconstruct):
+ *   rho[j] = rho~(E_j);  fvac[k][j] = rho~ C_vv(E_j,t_k);  fmsd[k][j] = rho~ DeltaX^2(E_j,t_k).
+ * With the paper's rho = dens * rho~, dens = 2N/Omega (nm^-2 for a 2-D sample; eq 8),
+ * in units of e^2/h:
+ *   sigma_gk = 2 pi hbar dens * int_0^t rho~C_vv dt'         (eq 6; trapezoid rule)
+ *   sigma_e1 = 2 pi hbar dens * (1/2) d(rho~DX2)/dt          (eq 9; central differences,
+ *                                                             second-order one-sided at both ends)
+ *   sigma_e2 = 2 pi hbar dens * rho~DX2 / (2 t), 0 at t = 0  (eq 11)
+ *   length_nm = 2 sqrt(fmsd / rho)                           (eq 50)
+ *   conductance = (width_nm / length_nm) * sigma_e1, 0 where the length is 0  (eq 51)
+ * All arrays fp64, host or device; tables are [n_steps+1][n_energies].  Every output pointer may
+ * be NULL; fvac (fmsd, rho) may be NULL when no requested output needs it.  Synchronises `stream`.
+ */
+int kg_transport(int n_steps, int n_energies, double dt_fs, double dens_per_nm2, double width_nm,
+                 const double *rho, const double *fvac, const double *fmsd, double *sigma_gk,
+                 double *sigma_e1, double *sigma_e2, double *length_nm, double *conductance,
+                 void *stream);
+
 /* Tuning / introspection (not part of the paper's problem statement). */
 enum {
     KG_OPT_USE_GRAPHS = 1,   /* 1 (default): replay the moment loop as a CUDA graph */

@@ -505,3 +505,56 @@ void kgo_kpm_reconstruct(int M, const kgo_c *mu, int use_jackson, double e0, dou
     }
     free(g);
 }
+
+/* ------------------------------------------------------------------------- */
+/* O10. Running conductivities and ballistic conductance from reconstructed   */
+/* functions of (t_k, E_j), t_k = k dt, k = 0..nt (reading g8):               */
+/*   rho[j]      = rho~(E_j)               (eq 29, per site and spin, 1/eV)   */
+/*   fvac[k][j]  = rho~ C_vv(E_j, t_k)     (eq 30, nm^2/fs^2/eV)              */
+/*   fmsd[k][j]  = rho~ DeltaX^2(E_j,t_k)  (eq 31, nm^2/eV)                   */
+/* The paper's rho = dens * rho~ with dens = 2N/Omega (2 = spin, eq 8,   */
+/* <phi|phi> = N P:128), so in units of e^2/h (h = 2 pi hbar):                */
+/*   sigma_GK(E,t) = 2 pi hbar dens int_0^t rho~C_vv dt'      (eq 6  P:61)    */
+/*   sigma_E1(E,t) = 2 pi hbar dens (1/2) d(rho~DX2)/dt       (eq 9  P:71)    */
+/*   sigma_E2(E,t) = 2 pi hbar dens rho~DX2 / (2t), 0 at t=0  (eq 11)    */
+/*   L(E,t)        = 2 sqrt(DX2) = 2 sqrt(fmsd/rho)           (eq 50)   */
+/*   G(E,t)        = (W/L) sigma_E1, 0 where L = 0            (eq 51)   */
+/* Discretisation (reading g14; the paper is silent): trapezoid rule for the  */
+/* integral; central differences for the derivative, second-order one-sided   */
+/* three-point formulas at k = 0 and k = nt (two-point when nt = 1).          */
+/* Any output pointer may be NULL; fvac / fmsd may be NULL if unused.         */
+/* ------------------------------------------------------------------------- */
+static double kgo_ddt(const double *f, int k, int nt, int ne, int j, double dt)
+{
+    if (nt < 1) return 0.0;
+    if (nt == 1) return (f[1 * ne + j] - f[0 * ne + j]) / dt;
+    if (k == 0) return (-3.0 * f[0 * ne + j] + 4.0 * f[1 * ne + j] - f[2 * ne + j]) / (2.0 * dt);
+    if (k == nt)
+        return (3.0 * f[nt * ne + j] - 4.0 * f[(nt - 1) * ne + j] + f[(nt - 2) * ne + j]) / (2.0 * dt);
+    return (f[(k + 1) * ne + j] - f[(k - 1) * ne + j]) / (2.0 * dt);
+}
+
+void kgo_transport(int nt, int ne, double dt_fs, double dens_per_nm2, double width_nm,
+                   const double *rho, const double *fvac, const double *fmsd, double *sigma_gk,
+                   double *sigma_e1, double *sigma_e2, double *length_nm, double *conductance)
+{
+    const double pref = 2.0 * M_PI * KGO_HBAR * dens_per_nm2;
+    for (int j = 0; j < ne; ++j) {
+        long double integral = 0.0L;
+        for (int k = 0; k <= nt; ++k) {
+            if (sigma_gk) {
+                if (k > 0)
+                    integral += 0.5L * ((long double)fvac[(k - 1) * ne + j] + fvac[k * ne + j]) * dt_fs;
+                sigma_gk[k * ne + j] = pref * (double)integral;
+            }
+            if (!fmsd) continue;
+            const double e1 = pref * 0.5 * kgo_ddt(fmsd, k, nt, ne, j, dt_fs);
+            if (sigma_e1) sigma_e1[k * ne + j] = e1;
+            if (sigma_e2) sigma_e2[k * ne + j] = k == 0 ? 0.0 : pref * fmsd[k * ne + j] / (2.0 * k * dt_fs);
+            const double dx2 = fmsd[k * ne + j] / rho[j];
+            const double len = 2.0 * sqrt(dx2 > 0.0 ? dx2 : 0.0);
+            if (length_nm) length_nm[k * ne + j] = len;
+            if (conductance) conductance[k * ne + j] = len > 0.0 ? width_nm / len * e1 : 0.0;
+        }
+    }
+}

@@ -229,3 +229,20 @@ def kpm_reconstruct(mu, e0, s, energies, use_jackson=True):
     lib().kgo_kpm_reconstruct(C.c_int(mu.shape[0]), _p(mu), C.c_int(int(use_jackson)),
                               C.c_double(e0), C.c_double(s), C.c_int(en.shape[0]), _p(en), _p(f))
     return f
+
+
+def transport(rho, fvac, fmsd, dt_fs, dens_per_nm2, width_nm=1.0):
+    """O10: dict of sigma_gk, sigma_e1, sigma_e2, length_nm, conductance ([nt+1][ne] each, in e^2/h
+    resp. nm) from rho [ne], fvac / fmsd [nt+1][ne] (either may be None)."""
+    rho = _f64(rho)
+    ref = fvac if fvac is not None else fmsd
+    nt, ne = ref.shape[0] - 1, ref.shape[1]
+    fv = None if fvac is None else _f64(fvac)
+    fm = None if fmsd is None else _f64(fmsd)
+    out = {}
+    for name, need in (("sigma_gk", fv), ("sigma_e1", fm), ("sigma_e2", fm), ("length_nm", fm), ("conductance", fm)):
+        out[name] = None if need is None else np.empty((nt + 1, ne))
+    lib().kgo_transport(C.c_int(nt), C.c_int(ne), C.c_double(dt_fs), C.c_double(dens_per_nm2),
+                        C.c_double(width_nm), _p(rho), _p(fv), _p(fm), _p(out["sigma_gk"]),
+                        _p(out["sigma_e1"]), _p(out["sigma_e2"]), _p(out["length_nm"]), _p(out["conductance"]))
+    return out

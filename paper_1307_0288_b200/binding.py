@@ -49,6 +49,7 @@ _lib.kg_vac.argtypes = [_vp, _vp, _int, _int, _int, _dbl, _dbl, _vp, _vp]
 _lib.kg_msd.argtypes = [_vp, _vp, _int, _int, _int, _dbl, _dbl, _vp, _vp]
 _lib.kg_bessel_terms.argtypes = [_dbl, _dbl, C.POINTER(_int), _vp, _int]
 _lib.kg_set_option.argtypes = [_vp, _int, _i64]
+_lib.kg_transport.argtypes = [_int, _int, _dbl, _dbl, _dbl] + [_vp] * 9
 _lib.kg_kpm_reconstruct.argtypes = [_vp, _i64, _int, _int, _dbl, _dbl, _vp, _int, _vp, _vp]
 
 
@@ -237,3 +238,24 @@ def kpm_reconstruct(mu, e0_eV, scale_eV, energies_eV, jackson=True, stream=None)
     _check(_lib.kg_kpm_reconstruct(_ptr(mu), rows, M, int(bool(jackson)), float(e0_eV), float(scale_eV),
                                    _ptr(energies_eV), ne, _ptr(f), _stream(stream)))
     return f
+
+
+def transport(rho, fvac, fmsd, dt_fs, dens_per_nm2, width_nm=1.0, stream=None):
+    """kg_transport: dict of sigma_gk (needs fvac), sigma_e1, sigma_e2, length_nm, conductance
+    (need fmsd) as [n_steps+1][n_energies] arrays of the same kind as the inputs (eqs 6-11, 50-51)."""
+    ref = fvac if fvac is not None else fmsd
+    nt, ne = int(ref.shape[0]) - 1, int(ref.shape[1])
+
+    def new():
+        if isinstance(ref, np.ndarray):
+            return np.empty((nt + 1, ne), np.float64)
+        return torch.empty((nt + 1, ne), dtype=torch.float64, device=ref.device)
+    out = {"sigma_gk": new() if fvac is not None else None}
+    for k in ("sigma_e1", "sigma_e2"):
+        out[k] = new() if fmsd is not None else None
+    for k in ("length_nm", "conductance"):                 # eq 50-51 need rho~ as well
+        out[k] = new() if fmsd is not None and rho is not None else None
+    _check(_lib.kg_transport(nt, ne, float(dt_fs), float(dens_per_nm2), float(width_nm), _ptr(rho), _ptr(fvac),
+                             _ptr(fmsd), _ptr(out["sigma_gk"]), _ptr(out["sigma_e1"]), _ptr(out["sigma_e2"]),
+                             _ptr(out["length_nm"]), _ptr(out["conductance"]), _stream(stream)))
+    return out

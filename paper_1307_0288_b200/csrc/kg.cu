@@ -993,3 +993,41 @@ extern "C" int kg_kpm_reconstruct(const kg_c128 *mu, int64_t rows, int M, int ja
     CUDA_TRY(cudaStreamSynchronize(st));     // temporaries are freed on return
     return KG_OK;
 }
+
+extern "C" int kg_transport(int n_steps, int n_energies, double dt_fs, double dens_per_nm2, double width_nm,
+                            const double *rho, const double *fvac, const double *fmsd, double *sigma_gk,
+                            double *sigma_e1, double *sigma_e2, double *length_nm, double *conductance,
+                            void *stream)
+{
+    if (n_steps < 0 || n_energies < 1) return fail(KG_EINVAL, "kg_transport: n_steps >= 0, n_energies >= 1");
+    if (!(dt_fs > 0.0) || !std::isfinite(dt_fs) || !std::isfinite(dens_per_nm2) || !std::isfinite(width_nm))
+        return fail(KG_EINVAL, "kg_transport: dt_fs must be positive; dens and width finite");
+    if (sigma_gk && !fvac) return fail(KG_EINVAL, "kg_transport: sigma_gk needs fvac");
+    if ((sigma_e1 || sigma_e2 || length_nm || conductance) && !fmsd)
+        return fail(KG_EINVAL, "kg_transport: sigma_e1 / sigma_e2 / length / conductance need fmsd");
+    if ((length_nm || conductance) && !rho) return fail(KG_EINVAL, "kg_transport: length / conductance need rho");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t tbytes = (size_t)(n_steps + 1) * n_energies * 8;
+    TmpDev tmp;
+    const void *d_rho, *d_vac, *d_msd;
+    int rc;
+    if ((rc = tmp.get(rho, (size_t)n_energies * 8, st, &d_rho)) || (rc = tmp.get(sigma_gk ? fvac : nullptr, tbytes, st, &d_vac)) ||
+        (rc = tmp.get(fmsd, tbytes, st, &d_msd)))
+        return rc;
+    double *user[5] = {sigma_gk, sigma_e1, sigma_e2, length_nm, conductance};
+    double *dev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    for (int q = 0; q < 5; ++q) {
+        if (!user[q]) continue;
+        if (is_device_ptr(user[q])) { dev[q] = user[q]; continue; }
+        CUDA_TRY(cudaMalloc(&dev[q], tbytes));
+        tmp.ptrs.push_back(dev[q]);
+    }
+    kg_transport_kernel<<<(n_energies + 127) / 128, 128, 0, st>>>(n_steps, n_energies, dt_fs,
+        2.0 * 3.14159265358979323846 * KG_HBAR * dens_per_nm2, width_nm, (const double *)d_rho,
+        (const double *)d_vac, (const double *)d_msd, dev[0], dev[1], dev[2], dev[3], dev[4]);
+    CUDA_TRY(cudaGetLastError());
+    for (int q = 0; q < 5; ++q)
+        if (user[q] && dev[q] != user[q]) CUDA_TRY(cudaMemcpyAsync(user[q], dev[q], tbytes, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return KG_OK;
+}

@@ -403,3 +403,50 @@ __global__ void kg_kpm_reconstruct_kernel(const c128 *__restrict__ mu, int64_t r
     }
     f[row * (int64_t)ne + j] = sum / (3.14159265358979323846 * s * sqrt(1.0 - x * x));
 }
+
+// ---------------------------------------------------------------------------------------
+// Running conductivities (eqs 6, 9, 11 P:61-78) and ballistic length / conductance (eqs 50-51
+// P:496-501) from reconstructed rho~(E_j), rho~C_vv(E_j,t_k), rho~DX2(E_j,t_k); one thread per
+// energy, time loop in order.  Trapezoid integral; central differences, second-order one-sided
+// at the two ends (reading g14).  Units of e^2/h: pref = 2 pi hbar * dens.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ double kg_ddt(const double *f, int k, int nt, int ne, int j, double dt)
+{
+    if (nt < 1) return 0.0;
+    if (nt == 1) return (f[ne + j] - f[j]) / dt;
+    if (k == 0) return (-3.0 * f[j] + 4.0 * f[ne + j] - f[2 * ne + j]) / (2.0 * dt);
+    if (k == nt)
+        return (3.0 * f[(int64_t)nt * ne + j] - 4.0 * f[(int64_t)(nt - 1) * ne + j] + f[(int64_t)(nt - 2) * ne + j]) / (2.0 * dt);
+    return (f[(int64_t)(k + 1) * ne + j] - f[(int64_t)(k - 1) * ne + j]) / (2.0 * dt);
+}
+
+__global__ void kg_transport_kernel(int nt, int ne, double dt, double pref, double width,
+                                    const double *__restrict__ rho, const double *__restrict__ fvac,
+                                    const double *__restrict__ fmsd, double *sigma_gk, double *sigma_e1,
+                                    double *sigma_e2, double *length_nm, double *conductance)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= ne) return;
+    double integral = 0.0, comp = 0.0;
+    for (int k = 0; k <= nt; ++k) {
+        const int64_t o = (int64_t)k * ne + j;
+        if (sigma_gk) {
+            if (k > 0) {
+                const double term = 0.5 * (fvac[o - ne] + fvac[o]) * dt - comp;
+                const double ns = integral + term;
+                comp = (ns - integral) - term;
+                integral = ns;
+            }
+            sigma_gk[o] = pref * integral;
+        }
+        if (!fmsd) continue;
+        const double e1 = pref * 0.5 * kg_ddt(fmsd, k, nt, ne, j, dt);
+        if (sigma_e1) sigma_e1[o] = e1;
+        if (sigma_e2) sigma_e2[o] = k == 0 ? 0.0 : pref * fmsd[o] / (2.0 * k * dt);
+        if (!length_nm && !conductance) continue;
+        const double dx2 = fmsd[o] / rho[j];
+        const double len = 2.0 * sqrt(dx2 > 0.0 ? dx2 : 0.0);
+        if (length_nm) length_nm[o] = len;
+        if (conductance) conductance[o] = len > 0.0 ? width / len * e1 : 0.0;
+    }
+}

@@ -340,3 +340,35 @@ def test_kpm_reconstruct(B, kgo, jackson):
     with pytest.raises(B.KgError) as e:
         B.kpm_reconstruct(mu, cfg.e0, cfg.scale, np.array([0.0, cfg.scale]), jackson)
     assert e.value.code == B.KG_EINVAL
+
+
+def test_transport_config2_like(B, kgo):
+    """The whole post-processing chain of config 2 on a scaled-down twin (50x50 cells, 0.5 %
+    vacancies): moments -> rho~, rho~C_vv, rho~DX2 on a 501-point grid -> sigma_GK, sigma_E1,
+    sigma_E2, L, G, every table against the oracle's own chain; device and host pointers."""
+    cfg = W.make_config(2, shrink=5)
+    lat = cfg.lattice
+    olat = to_oracle_lattice(kgo, lat)
+    h = B.from_lattice(lat, cfg.xcoord, cfg.period, cfg.e0, cfg.scale)
+    phi = W.random_phase_vectors(lat.n, 1, cfg.seed)
+    M, nt = 128, 6
+    en = W.energy_grid(501)
+    d_en = dev(en)
+    rho = B.kpm_reconstruct(B.dos_moments(h, dev(phi), M), cfg.e0, cfg.scale, d_en)[0]
+    fvac = B.kpm_reconstruct(B.vac(h, dev(phi), M, nt, cfg.dt_fs), cfg.e0, cfg.scale, d_en)[0]
+    fmsd = B.kpm_reconstruct(B.msd(h, dev(phi), M, nt, cfg.dt_fs), cfg.e0, cfg.scale, d_en)[0]
+    dens = 8.0 / (3 * np.sqrt(3) * 0.142 ** 2)             # 2N/Omega of graphene, nm^-2
+    got = B.transport(rho, fvac, fmsd, cfg.dt_fs, dens, 2.0)
+    v = phi[:, 0].copy()
+    orho = kgo.kpm_reconstruct(kgo.dos_moments(olat, cfg.e0, cfg.scale, v, M), cfg.e0, cfg.scale, en)
+    ovac = kgo.vac(olat, cfg.xcoord, cfg.period, cfg.e0, cfg.scale, v, M, nt, cfg.dt_fs)
+    omsd = kgo.msd(olat, cfg.xcoord, cfg.period, cfg.e0, cfg.scale, v, M, nt, cfg.dt_fs)
+    ofvac = np.stack([kgo.kpm_reconstruct(ovac[k], cfg.e0, cfg.scale, en) for k in range(nt + 1)])
+    ofmsd = np.stack([kgo.kpm_reconstruct(omsd[k], cfg.e0, cfg.scale, en) for k in range(nt + 1)])
+    want = kgo.transport(orho, ofvac, ofmsd, cfg.dt_fs, dens, 2.0)
+    for key in ("sigma_gk", "sigma_e1", "sigma_e2", "length_nm", "conductance"):
+        assert relerr(host(got[key]), want[key]) <= 1e-9, key
+    # host pointers, subset of outputs
+    hg = B.transport(None, None, host(fmsd), cfg.dt_fs, dens)
+    assert hg["sigma_gk"] is None
+    assert relerr(hg["sigma_e2"], want["sigma_e2"]) <= 1e-9

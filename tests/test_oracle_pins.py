@@ -425,3 +425,75 @@ def test_pristine_graphene_dos_closed_form(kgo):
     xk = np.cos(np.pi * (np.arange(K) + 0.5) / K)
     f = kgo.kpm_reconstruct(mu, 0.0, S_GRAPHENE, xk * S_GRAPHENE)
     assert abs(np.sum(np.pi / K * np.sqrt(1 - xk**2) * f) * S_GRAPHENE - 1.0) < 1e-12
+
+
+# ------------------------------------------------------------------ transport post-processing (O10)
+def _chain_closed_forms(en, t=2.7, a=0.142):
+    """Infinite 1-D chain, per site and spin: rho~ = 1/(pi sqrt(4t^2 - E^2)); E = 2t cos(ka),
+    v = (2ta/hbar) sin(ka) => v^2(E) = (a/hbar)^2 (4t^2 - E^2).  Textbook results."""
+    root = np.sqrt(4 * t * t - en ** 2)
+    return 1.0 / (np.pi * root), (a / HBAR) ** 2 * root ** 2
+
+
+def test_transport_ballistic_closed_forms(kgo):
+    """Ballistic inputs rho~ v^2 (VAC) and rho~ v^2 t^2 (MSD) of the 1-D chain: sigma_GK = sigma_E1
+    (P:532), sigma_E2 = sigma_E1 / 2, L = 2 v t (eq 50), and the Landauer value: one open
+    channel, G = 2e^2/h = 2 in units of e^2/h, at every energy in the band and every t > 0 (eq 51,
+    52).  A wrong prefactor, a dropped 1/2, a first-order end-point derivative or a wrong
+    trapezoid weight breaks one of these."""
+    a, nt, dt = 0.142, 7, 0.37
+    en = np.linspace(-5.0, 5.0, 41)
+    rho, v2 = _chain_closed_forms(en, a=a)
+    tk = dt * np.arange(nt + 1)[:, None]
+    fvac = np.broadcast_to(rho * v2, (nt + 1, en.size)).copy()
+    fmsd = rho * v2 * tk ** 2
+    width = 1.0                                   # strip of width 1 nm: Omega = W N a, dens = 2N/Omega
+    out = kgo.transport(rho, fvac, fmsd, dt, 2.0 / (a * width), width)
+    assert relerr(out["sigma_e1"], out["sigma_gk"]) < 1e-13
+    assert relerr(out["sigma_e2"][1:], 0.5 * out["sigma_e1"][1:]) < 1e-13
+    assert np.all(out["sigma_e2"][0] == 0)
+    assert relerr(out["length_nm"], 2 * np.sqrt(v2) * tk) < 1e-13
+    assert np.max(np.abs(out["conductance"][1:] - 2.0)) < 1e-12
+    assert np.all(out["conductance"][0] == 0)
+    # absolute value of sigma: 2 pi hbar dens rho~ v^2 t
+    assert relerr(out["sigma_gk"], 2 * np.pi * HBAR * (2.0 / a) * rho * v2 * tk) < 1e-13
+
+
+def test_transport_diffusive_and_quadrature(kgo):
+    """Diffusive MSD 2 D t: sigma_E1 = sigma_E2 = 2 pi hbar dens rho D, independent of t; and the
+    Green-Kubo integral of an exponentially decaying VAC within the trapezoid error bound."""
+    nt, dt, dens, D, tau = 40, 0.05, 38.2, 0.6, 0.9
+    rho = np.array([0.01, 0.05, 0.11])
+    tk = dt * np.arange(nt + 1)[:, None]
+    out = kgo.transport(rho, None, rho * 2 * D * tk, dt, dens)
+    want = 2 * np.pi * HBAR * dens * rho * D
+    assert out["sigma_gk"] is None
+    assert relerr(out["sigma_e1"], np.broadcast_to(want, (nt + 1, 3))) < 1e-12
+    assert relerr(out["sigma_e2"][1:], np.broadcast_to(want, (nt, 3))) < 1e-12
+    fvac = rho * (D / tau) * np.exp(-tk / tau)
+    gk = kgo.transport(rho, fvac, None, dt, dens)["sigma_gk"]
+    exact = 2 * np.pi * HBAR * dens * rho * D * (1 - np.exp(-tk / tau))
+    bound = 2 * np.pi * HBAR * dens * rho * (D / tau ** 3) * dt ** 2 / 12 * tk      # |f''| t dt^2 / 12
+    assert np.all(np.abs(gk - exact) <= bound + 1e-15)
+    assert np.max(np.abs(gk - exact)) > 0                                            # really a quadrature
+
+
+def test_transport_end_to_end_ring_conductance(kgo):
+    """The whole Einstein chain of the oracle on a pristine ring (Alg. 3 -> eq 31 -> eqs 9, 50, 51):
+    one ballistic channel, G = 1 in units of 2e^2/h inside the band (P:515-524 plateaus)."""
+    n, t, a = 3000, 2.7, 0.142
+    lat = ring(kgo, n, -t, a)
+    s = 2 * t * 1.05
+    # a state on one site: on the translation-invariant ring <0|A delta(E-H) A|0> = Tr[...]/N
+    # exactly, so there is no stochastic error, only the Jackson broadening pi s/M = 0.11 eV
+    phi = np.zeros(n, complex); phi[0] = 1.0
+    M, nt, dt = 160, 6, 2 * HBAR / t
+    en = np.linspace(-1.5 * t, 1.5 * t, 31)
+    rho = kgo.kpm_reconstruct(kgo.dos_moments(lat, 0.0, s, phi, M), 0.0, s, en)
+    mu = kgo.msd(lat, lat.x, lat.period_x, 0.0, s, phi, M, nt, dt)
+    fmsd = np.stack([kgo.kpm_reconstruct(mu[k], 0.0, s, en) for k in range(nt + 1)])
+    out = kgo.transport(rho, None, fmsd, dt, 2.0 / a, 1.0)
+    g = out["conductance"][1:] / 2.0                      # in 2e^2/h
+    print("ring conductance / (2e^2/h): mean %.6f, max dev %.2e" % (np.mean(g), np.max(np.abs(g - 1.0))))
+    assert abs(np.mean(g) - 1.0) < 5e-4
+    assert np.max(np.abs(g - 1.0)) < 1e-3
