@@ -209,6 +209,28 @@ int kg_transport(int n_steps, int n_energies, double dt_fs, double dens_per_nm2,
                  double *sigma_e1, double *sigma_e2, double *length_nm, double *conductance,
                  void *stream);
 
+/*
+ * kg_fourier_moments — Fourier moments F_n = <phi_L| U(n dtau) |phi_R>, n = -Nm..Nm (Alg. 4
+ * P:320-344, eq 45; eqs 25-27): phi' <- phi_R, then Nm applications of U(dtau) (Alg. 6, as
+ * kg_evolve) with an inner product after each, and the same with U^dagger(dtau) for n < 0.
+ *   phiL, phiR [n][R] (may be the same pointer);  F [R][2*Nm+1] complex128, F_n of vector r at
+ *   F[r*(2*Nm+1) + n + Nm];  dtau_fs > 0 (the paper's choice: pi hbar / s);  Nm >= 0.
+ * Inner products use per-block partials and a fixed-order final sum (bitwise reproducible).
+ */
+int kg_fourier_moments(kg_hamiltonian *h, const kg_c128 *phiL, const kg_c128 *phiR, int R, int Nm,
+                       double dtau_fs, double bessel_eps, kg_c128 *F, void *stream);
+
+/*
+ * kg_ftm_reconstruct — Fourier-transform-method reconstruction (eqs 22-24) with the
+ * Hanning window w_n = (1 + cos(pi n/(Nm+1)))/2 (eq 28; window = 0: w_n = 1), per site
+ * and spin for unit-norm phi:
+ *   f[row][j] = dtau/(2 pi hbar) * sum_{n=-Nm}^{Nm} w_n Re[ exp(i E_j n dtau/hbar) F[row][n+Nm] ].
+ *   F [rows][2*Nm+1], energies_eV [n_energies], f [rows][n_energies]; host or device pointers.
+ * Synchronises `stream` before returning.
+ */
+int kg_ftm_reconstruct(const kg_c128 *F, int64_t rows, int Nm, int window, double dtau_fs,
+                       const double *energies_eV, int n_energies, double *f, void *stream);
+
 /* Tuning / introspection (not part of the paper's problem statement). */
 enum {
     KG_OPT_USE_GRAPHS = 1,   /* 1 (default): replay the moment loop as a CUDA graph */

@@ -558,3 +558,51 @@ void kgo_transport(int nt, int ne, double dt_fs, double dens_per_nm2, double wid
         }
     }
 }
+
+/* ------------------------------------------------------------------------- */
+/* O11. Fourier moments (Alg. 4; eq 45; eqs 25-27):  */
+/*   F_n = <phi_L| U(n dtau) |phi_R>,  n = -Nm..Nm,  stored at F[n + Nm].      */
+/* l.1-6: phi' <- phi_R, F_0, then phi' <- U(dtau) phi' and F_n for n = 1..Nm; */
+/* l.7-11: the same with U^dagger(dtau) for F_{-n}.  U by Alg. 6 (kgo_evolve). */
+/* ------------------------------------------------------------------------- */
+int kgo_fourier_moments(int64_t n, int kmax, const int32_t *nn, const int32_t *nl, const double *hop,
+                        const double *onsite, double e0, double s, const kgo_c *phiL,
+                        const kgo_c *phiR, int Nm, double dtau_fs, double eps, kgo_c *F)
+{
+    kgo_c *a = (kgo_c *)malloc((size_t)n * sizeof(kgo_c));
+    kgo_c *b = (kgo_c *)malloc((size_t)n * sizeof(kgo_c));
+    if (!a || !b) { free(a); free(b); return 1; }
+    for (int dir = +1; dir >= -1; dir -= 2) {
+        memcpy(a, phiR, (size_t)n * sizeof(kgo_c));                       /* l.1 / l.7 */
+        if (dir > 0) F[Nm] = kgo_dot(n, phiL, a);                         /* l.2 */
+        for (int m = 1; m <= Nm; ++m) {                                   /* l.3 / l.8 */
+            if (kgo_evolve(n, kmax, nn, nl, hop, onsite, e0, s, a, dir * dtau_fs, eps, b)) {
+                free(a); free(b); return 1;
+            }
+            kgo_c *t = a; a = b; b = t;                                   /* l.4 / l.9 */
+            F[Nm + dir * m] = kgo_dot(n, phiL, a);                        /* l.5 / l.10 */
+        }
+    }
+    free(a); free(b);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------- */
+/* O12. FTM reconstruction (eqs 22-24) with the Hanning window       */
+/* w_n = (1 + cos(pi n/(Nm+1)))/2 (eq 28), per site and spin for a   */
+/* unit-norm phi (the paper's (2/Omega) Tr -> <phi|.|phi>, readings g1, g3):   */
+/*   f(E) = dtau/(2 pi hbar) sum_{n=-Nm}^{Nm} w_n Re[ e^{i E n dtau/hbar} F_n ]  */
+/* (delta(E-H) = (1/2 pi hbar) int dt e^{i(E-H)t/hbar}, discretised with dtau). */
+/* ------------------------------------------------------------------------- */
+void kgo_ftm_reconstruct(int Nm, const kgo_c *F, int use_window, double dtau_fs, int ne,
+                         const double *energies, double *f)
+{
+    for (int j = 0; j < ne; ++j) {
+        long double sum = 0.0L;
+        for (int m = -Nm; m <= Nm; ++m) {
+            const double w = use_window ? 0.5 * (1.0 + cos(M_PI * m / (Nm + 1.0))) : 1.0;
+            sum += (long double)(w * creal(cexp(I * energies[j] * m * dtau_fs / KGO_HBAR) * F[m + Nm]));
+        }
+        f[j] = (double)sum * dtau_fs / (2.0 * M_PI * KGO_HBAR);
+    }
+}

@@ -246,3 +246,22 @@ def transport(rho, fvac, fmsd, dt_fs, dens_per_nm2, width_nm=1.0):
                         C.c_double(width_nm), _p(rho), _p(fv), _p(fm), _p(out["sigma_gk"]),
                         _p(out["sigma_e1"]), _p(out["sigma_e2"]), _p(out["length_nm"]), _p(out["conductance"]))
     return out
+
+
+def fourier_moments(lat, e0, s, phiL, phiR, Nm, dtau_fs, eps=1e-15):
+    """O11 (Alg. 4): F[n + Nm] = <phiL|U(n dtau)|phiR>, n = -Nm..Nm."""
+    phiL = _c128(phiL); phiR = _c128(phiR); F = np.empty(2 * Nm + 1, np.complex128)
+    rc = lib().kgo_fourier_moments(*_lat_args(lat), _p(lat.onsite), C.c_double(e0), C.c_double(s),
+                                   _p(phiL), _p(phiR), C.c_int(Nm), C.c_double(dtau_fs),
+                                   C.c_double(eps), _p(F))
+    assert rc == 0
+    return F
+
+
+def ftm_reconstruct(F, dtau_fs, energies, use_window=True):
+    """O12 (eqs 22-24, 28): f(E) from Fourier moments F[n + Nm]."""
+    F = _c128(F); en = _f64(energies); f = np.empty(en.shape[0])
+    Nm = (F.shape[0] - 1) // 2
+    lib().kgo_ftm_reconstruct(C.c_int(Nm), _p(F), C.c_int(int(use_window)), C.c_double(dtau_fs),
+                              C.c_int(en.shape[0]), _p(en), _p(f))
+    return f

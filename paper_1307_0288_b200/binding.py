@@ -50,6 +50,8 @@ _lib.kg_msd.argtypes = [_vp, _vp, _int, _int, _int, _dbl, _dbl, _vp, _vp]
 _lib.kg_bessel_terms.argtypes = [_dbl, _dbl, C.POINTER(_int), _vp, _int]
 _lib.kg_set_option.argtypes = [_vp, _int, _i64]
 _lib.kg_transport.argtypes = [_int, _int, _dbl, _dbl, _dbl] + [_vp] * 9
+_lib.kg_fourier_moments.argtypes = [_vp, _vp, _vp, _int, _int, _dbl, _dbl, _vp, _vp]
+_lib.kg_ftm_reconstruct.argtypes = [_vp, _i64, _int, _int, _dbl, _vp, _int, _vp, _vp]
 _lib.kg_kpm_reconstruct.argtypes = [_vp, _i64, _int, _int, _dbl, _dbl, _vp, _int, _vp, _vp]
 
 
@@ -259,3 +261,29 @@ def transport(rho, fvac, fmsd, dt_fs, dens_per_nm2, width_nm=1.0, stream=None):
                              _ptr(fmsd), _ptr(out["sigma_gk"]), _ptr(out["sigma_e1"]), _ptr(out["sigma_e2"]),
                              _ptr(out["length_nm"]), _ptr(out["conductance"]), _stream(stream)))
     return out
+
+
+def fourier_moments(h: Hamiltonian, phiL, phiR, Nm, dtau_fs, bessel_eps=1e-15, F=None, stream=None):
+    """kg_fourier_moments (Alg. 4): F[r, n + Nm] = <phiL_r|U(n dtau)|phiR_r>, n = -Nm..Nm."""
+    phiR, R = _vec(phiR, h.n)
+    phiL, RL = _vec(phiL, h.n)
+    assert R == RL
+    if F is None:
+        F = _empty_like_mu(phiR, (R, 2 * Nm + 1))
+    _check(_lib.kg_fourier_moments(h._h, _ptr(phiL), _ptr(phiR), R, Nm, dtau_fs, bessel_eps, _ptr(F), _stream(stream)))
+    return F
+
+
+def ftm_reconstruct(F, dtau_fs, energies_eV, window=True, stream=None):
+    """kg_ftm_reconstruct: F [..., 2Nm+1] -> f [..., n_energies] (eqs 22-24, 28)."""
+    Nm = (int(F.shape[-1]) - 1) // 2
+    lead = tuple(F.shape[:-1])
+    rows = int(np.prod(lead)) if lead else 1
+    ne = int(energies_eV.shape[0])
+    if isinstance(F, np.ndarray):
+        f = np.empty(lead + (ne,), np.float64)
+    else:
+        f = torch.empty(lead + (ne,), dtype=torch.float64, device=F.device)
+    _check(_lib.kg_ftm_reconstruct(_ptr(F), rows, Nm, int(bool(window)), float(dtau_fs), _ptr(energies_eV), ne,
+                                   _ptr(f), _stream(stream)))
+    return f

@@ -1031,3 +1031,90 @@ extern "C" int kg_transport(int n_steps, int n_energies, double dt_fs, double de
     CUDA_TRY(cudaStreamSynchronize(st));
     return KG_OK;
 }
+
+// --------------------------------------------------------------------------------------
+// Fourier-transform method: Alg. 4 = kg_evolve in a loop + inner products
+// --------------------------------------------------------------------------------------
+static int dot_device(kg_hamiltonian *h, const c128 *a, int ld_a, const c128 *b, int R, c128 *partial,
+                      int grid, cudaStream_t st)
+{
+    switch (R) {
+    case 1: kg_dot_kernel<1><<<grid, 256, 0, st>>>(a, ld_a, b, h->n, partial); break;
+    case 2: kg_dot_kernel<2><<<grid, 256, 0, st>>>(a, ld_a, b, h->n, partial); break;
+    case 4: kg_dot_kernel<4><<<grid, 256, 0, st>>>(a, ld_a, b, h->n, partial); break;
+    case 8: kg_dot_kernel<8><<<grid, 256, 0, st>>>(a, ld_a, b, h->n, partial); break;
+    default: return fail(KG_EUNSUPPORTED, "R must be 1, 2, 4 or 8");
+    }
+    h->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return KG_OK;
+}
+
+extern "C" int kg_fourier_moments(kg_hamiltonian *h, const kg_c128 *phiL, const kg_c128 *phiR, int R, int Nm,
+                                  double dtau_fs, double bessel_eps, kg_c128 *F, void *stream)
+{
+    if (!h || !phiL || !phiR || !F) return fail(KG_EINVAL, "kg_fourier_moments: NULL argument");
+    if (!r_ok(R, false)) return fail(KG_EUNSUPPORTED, "R must be 1, 2, 4 or 8");
+    if (Nm < 0) return fail(KG_EINVAL, "Nm must be >= 0");
+    if (!(dtau_fs > 0.0) || !std::isfinite(dtau_fs)) return fail(KG_EINVAL, "dtau_fs must be finite and positive");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t vbytes = (size_t)h->n * R * 16;
+    const int rows = 2 * Nm + 1;
+    const int grid = grid_for(h, h->n * R);
+    const void *dL, *dR;
+    void *b0, *b1, *part;
+    OutStage o;
+    int rc;
+    if ((rc = stage_in(h, WS_IN0, phiL, vbytes, st, &dL))) return rc;
+    if (phiR == phiL) dR = dL;
+    else if ((rc = stage_in(h, WS_IN1, phiR, vbytes, st, &dR))) return rc;
+    if ((rc = ws_get(h, WS_S0, vbytes, &b0)) || (rc = ws_get(h, WS_S1, vbytes, &b1)) ||
+        (rc = ws_get(h, WS_PART, (size_t)rows * grid * R * 16, &part)) ||
+        (rc = stage_out(h, WS_MU, F, (size_t)R * rows * 16, &o)))
+        return rc;
+    const size_t prow = (size_t)grid * R;
+    c128 *P = (c128 *)part;
+    if ((rc = dot_device(h, (const c128 *)dL, R, (const c128 *)dR, R, P + (size_t)Nm * prow, grid, st))) return rc;   // l.2
+    for (int dir = +1; dir >= -1; dir -= 2) {
+        const c128 *cur = (const c128 *)dR;                                       // l.1 / l.7
+        c128 *nxt = (c128 *)b0;
+        for (int m = 1; m <= Nm; ++m) {
+            if ((rc = evolve_device(h, cur, R, nxt, R, dir * dtau_fs, bessel_eps, st)) ||             // l.4 / l.9
+                (rc = dot_device(h, (const c128 *)dL, R, nxt, R, P + (size_t)(Nm + dir * m) * prow, grid, st)))   // l.5 / l.10
+                return rc;
+            cur = nxt;
+            nxt = (nxt == (c128 *)b0) ? (c128 *)b1 : (c128 *)b0;
+        }
+    }
+    kg_reduce_partials<<<(rows * R * 32 + 255) / 256, 256, 0, st>>>(P, rows, grid, R, (c128 *)o.dev, rows, 0);
+    h->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return finish_out(o, st);
+}
+
+extern "C" int kg_ftm_reconstruct(const kg_c128 *F, int64_t rows, int Nm, int window, double dtau_fs,
+                                  const double *energies_eV, int n_energies, double *f, void *stream)
+{
+    if (!F || !energies_eV || !f) return fail(KG_EINVAL, "kg_ftm_reconstruct: NULL argument");
+    if (rows <= 0 || rows > 65535 || Nm < 0 || n_energies < 1)
+        return fail(KG_EINVAL, "kg_ftm_reconstruct: need 1 <= rows <= 65535, Nm >= 0, n_energies >= 1");
+    if (!(dtau_fs > 0.0) || !std::isfinite(dtau_fs)) return fail(KG_EINVAL, "dtau_fs must be finite and positive");
+    cudaStream_t st = (cudaStream_t)stream;
+    TmpDev tmp;
+    const void *d_F, *d_en;
+    int rc;
+    if ((rc = tmp.get(F, (size_t)rows * (2 * Nm + 1) * 16, st, &d_F)) ||
+        (rc = tmp.get(energies_eV, (size_t)n_energies * 8, st, &d_en)))
+        return rc;
+    double *d_f = nullptr;
+    const bool f_dev = is_device_ptr(f);
+    if (f_dev) d_f = f;
+    else { CUDA_TRY(cudaMalloc(&d_f, (size_t)rows * n_energies * 8)); tmp.ptrs.push_back(d_f); }
+    dim3 grid((n_energies + 127) / 128, (unsigned)rows);
+    kg_ftm_reconstruct_kernel<<<grid, 128, 0, st>>>((const c128 *)d_F, rows, Nm, window, dtau_fs / KG_HBAR,
+                                                    (const double *)d_en, n_energies, d_f);
+    CUDA_TRY(cudaGetLastError());
+    if (!f_dev) CUDA_TRY(cudaMemcpyAsync(f, d_f, (size_t)rows * n_energies * 8, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return KG_OK;
+}

@@ -450,3 +450,56 @@ __global__ void kg_transport_kernel(int nt, int ne, double dt, double pref, doub
         if (conductance) conductance[o] = len > 0.0 ? width / len * e1 : 0.0;
     }
 }
+
+// ---------------------------------------------------------------------------------------
+// Inner product kernel of Alg. 4 (l.2, 5, 10 P:325-341): per-block partial of <a|b> per vector,
+// a at a[i*ld_a + r], b at b[i*R + r]; finished by kg_reduce_partials (fixed order).
+// ---------------------------------------------------------------------------------------
+template <int R>
+__global__ void __launch_bounds__(256) kg_dot_kernel(const c128 *__restrict__ a, int ld_a,
+                                                      const c128 *__restrict__ b, int64_t n,
+                                                      c128 *__restrict__ partial)
+{
+    __shared__ c128 red[32 * R];
+    const int r = threadIdx.x & (R - 1);
+    c128 sum = make_double2(0.0, 0.0);
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n * R;
+         e += (int64_t)gridDim.x * blockDim.x) {
+        const c128 L = ld_nc(a + (e / R) * ld_a + r), v = ld_nc(b + e);
+        sum.x = fma(L.x, v.x, fma(L.y, v.y, sum.x));          // conj(a) * b
+        sum.y = fma(L.x, v.y, fma(-L.y, v.x, sum.y));
+    }
+    c128 tot = block_reduce_per_r<R>(sum, red);
+    if (threadIdx.x < R) partial[(int64_t)blockIdx.x * R + threadIdx.x] = tot;
+}
+
+// FTM reconstruction (eqs 22-24, Hanning window eq 28), per site and spin:
+// f[row][j] = dtau/(2 pi hbar) sum_{n=-Nm}^{Nm} w_n Re[e^{i E_j n dtau/hbar} F[row][n+Nm]].
+// The phase e^{i n x} is advanced by complex rotation and re-seeded from sincos every 32 terms.
+__global__ void kg_ftm_reconstruct_kernel(const c128 *__restrict__ F, int64_t rows, int Nm, int window,
+                                          double dtau_over_hbar, const double *__restrict__ energies,
+                                          int ne, double *__restrict__ f)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t row = blockIdx.y;
+    if (j >= ne || row >= rows) return;
+    const double x = energies[j] * dtau_over_hbar;
+    const c128 *Fr = F + row * (int64_t)(2 * Nm + 1) + Nm;
+    double sx, cx;
+    sincos(x, &sx, &cx);
+    double sum = Fr[0].x, comp = 0.0;                          // n = 0, w_0 = 1
+    double pr = 1.0, pi = 0.0;                                 // e^{i n x}
+    for (int n = 1; n <= Nm; ++n) {
+        if ((n & 31) == 0) sincos(n * x, &pi, &pr);
+        else { const double t = pr * cx - pi * sx; pi = pr * sx + pi * cx; pr = t; }
+        double w = 1.0;
+        if (window) w = 0.5 * (1.0 + cospi((double)n / (Nm + 1.0)));
+        // Re[e^{inx} F_n] + Re[e^{-inx} F_{-n}]
+        const c128 fp = Fr[n], fm = Fr[-n];
+        const double term = w * ((pr * fp.x - pi * fp.y) + (pr * fm.x + pi * fm.y)) - comp;
+        const double ns = sum + term;
+        comp = (ns - sum) - term;
+        sum = ns;
+    }
+    f[row * (int64_t)ne + j] = sum * dtau_over_hbar / (2.0 * 3.14159265358979323846);
+}

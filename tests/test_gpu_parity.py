@@ -372,3 +372,34 @@ def test_transport_config2_like(B, kgo):
     hg = B.transport(None, None, host(fmsd), cfg.dt_fs, dens)
     assert hg["sigma_gk"] is None
     assert relerr(hg["sigma_e2"], want["sigma_e2"]) <= 1e-9
+
+
+# --------------------------------------------------------------------------------- Fourier-transform method
+@pytest.mark.parametrize("R", [1, 4])
+def test_fourier_moments_and_ftm_reconstruct(B, kgo, R):
+    """Alg. 4 (F_n = <phi_L|U(n dtau)|phi_R>, n = -Nm..Nm) and eqs 22-24 + Hanning window on the
+    device against the oracle; distinct and identical left/right vectors; host pointers."""
+    lat = disordered()
+    e0 = 0.15
+    s = scale_for(lat, e0)
+    olat = to_oracle_lattice(kgo, lat)
+    h = B.from_lattice(lat, lat.x, lat.period_x, e0, s)
+    Nm, dtau = 12, np.pi * W.HBAR / s                       # P:474: dtau = pi hbar / s
+    L, Rv = rand_vectors(lat.n, R, 21), rand_vectors(lat.n, R, 22)
+    F = host(B.fourier_moments(h, dev(L), dev(Rv), Nm, dtau))
+    assert F.shape == (R, 2 * Nm + 1)
+    for r in range(R):
+        assert relerr(F[r], kgo.fourier_moments(olat, e0, s, L[:, r], Rv[:, r], Nm, dtau)) <= TOL
+    d = dev(Rv)
+    Fd = B.fourier_moments(h, d, d, Nm, dtau)               # DOS moments, eq 25
+    Fh = B.fourier_moments(h, Rv, Rv, Nm, dtau)             # host in -> host out
+    assert host(Fd).tobytes() == Fh.tobytes()
+    assert np.max(np.abs(Fh[:, Nm] - 1.0)) < 1e-13
+    assert np.max(np.abs(Fh[:, ::-1] - np.conj(Fh))) < 1e-12
+    en = np.linspace(-9.0, 9.0, 301)
+    for window in (True, False):
+        f = host(B.ftm_reconstruct(Fd, dtau, dev(en), window))
+        for r in range(R):
+            assert relerr(f[r], kgo.ftm_reconstruct(Fh[r], dtau, en, window)) <= TOL
+    f_host = B.ftm_reconstruct(Fh, dtau, en)
+    assert relerr(f_host, host(B.ftm_reconstruct(Fd, dtau, dev(en)))) <= 1e-13

@@ -497,3 +497,77 @@ def test_transport_end_to_end_ring_conductance(kgo):
     print("ring conductance / (2e^2/h): mean %.6f, max dev %.2e" % (np.mean(g), np.max(np.abs(g - 1.0))))
     assert abs(np.mean(g) - 1.0) < 5e-4
     assert np.max(np.abs(g - 1.0)) < 1e-3
+
+
+# ------------------------------------------------------------------ Fourier-transform method (O11, O12)
+@pytest.mark.parametrize("e0", [0.0, 0.3])
+def test_fourier_moments_vs_dense(kgo, e0):
+    """Alg. 4: F_n = sum_j conj(<j|phi_L>) <j|phi_R> exp(-i E_j n dtau/hbar), n = -Nm..Nm, from the
+    dense eigen-decomposition: pins the direction of time for +n / -n, the storage order, the
+    conjugated LEFT vector and the repeated application of U(dtau)."""
+    lat = small_disordered(kgo)
+    _, E, Vec = eig(lat)
+    s = (3 * 2.7 + 1.35 + abs(e0)) * 1.05
+    phiL, phiR = rand_state(lat.n, 14), rand_state(lat.n, 15)
+    cL, cR = Vec.T @ phiL, Vec.T @ phiR
+    Nm, dtau = 9, 0.21
+    nn_ = np.arange(-Nm, Nm + 1)
+    want = np.array([np.sum(np.conj(cL) * cR * np.exp(-1j * E * m * dtau / HBAR)) for m in nn_])
+    got = kgo.fourier_moments(lat, e0, s, phiL, phiR, Nm, dtau)
+    assert relerr(got, want) < 1e-12
+    same = kgo.fourier_moments(lat, e0, s, phiR, phiR, Nm, dtau)
+    assert np.max(np.abs(same[::-1] - np.conj(same))) < 1e-13          # F_{-n} = conj(F_n) if L = R
+    assert abs(same[Nm] - 1.0) < 1e-14
+
+
+def test_ftm_reconstruct_closed_forms(kgo):
+    """eqs 22-24 + Hanning window eq 28 on a single level E_a (F_n = exp(-i E_a n dtau/hbar)):
+    without window the Dirichlet kernel dtau/(2 pi hbar) sin((2Nm+1)x/2)/sin(x/2),
+    x = (E-E_a) dtau/hbar; with the window the peak value dtau (Nm+1)/(2 pi hbar) (sum of w_n);
+    and the integral over one period 2 pi hbar/dtau is w_0 F_0 = 1 in both cases."""
+    Nm, dtau, Ea = 12, 0.35, 0.8
+    nn_ = np.arange(-Nm, Nm + 1)
+    F = np.exp(-1j * Ea * nn_ * dtau / HBAR)
+    period = 2 * np.pi * HBAR / dtau
+    en = Ea + np.linspace(-0.5, 0.5, 400, endpoint=False) * period + 1e-3
+    x = (en - Ea) * dtau / HBAR
+    plain = kgo.ftm_reconstruct(F, dtau, en, use_window=False)
+    assert relerr(plain, dtau / (2 * np.pi * HBAR) * np.sin((2 * Nm + 1) * x / 2) / np.sin(x / 2)) < 1e-12
+    win = kgo.ftm_reconstruct(F, dtau, en, use_window=True)
+    peak = kgo.ftm_reconstruct(F, dtau, np.array([Ea]), use_window=True)[0]
+    assert abs(peak - dtau * (Nm + 1) / (2 * np.pi * HBAR)) < 1e-13
+    assert abs(np.min(win) / peak + 10 ** (-31.5 / 20)) < 1e-3          # Hann window: highest side lobe -31.5 dB (textbook)
+    assert np.min(plain) < -0.15 * np.max(plain)                        # Dirichlet: first side lobe -21 %
+    for f in (plain, win):                                              # uniform grid over one period:
+        assert abs(np.sum(f) * period / en.size - 1.0) < 1e-12          # exact for trig polynomials
+
+
+def test_ftm_and_kpm_dos_agree(kgo):
+    """The paper's own validation (Fig. 2): DOS of a disordered sheet by the FTM and by the
+    KPM from the same random vector, at a matched, coarse resolution; and both against the exact
+    levels broadened by the FTM window (dense diagonalisation)."""
+    full = kgo.honeycomb(8, 8)
+    lat = kgo.remove_sites(full, kgo.vacancy_mask(full.n, 6, 2))
+    s = S_GRAPHENE
+    _, E, Vec = eig(lat)
+    phi = rand_state(lat.n, 21)
+    dtau = np.pi * HBAR / s                                             # P:474: Delta tau = pi hbar / (Delta E / 2)
+    Nm = 40
+    en = np.linspace(-7.5, 7.5, 151)
+    F = kgo.fourier_moments(lat, 0.0, s, phi, phi, Nm, dtau)
+    ftm = kgo.ftm_reconstruct(F, dtau, en)
+    # exact: sum_j |<j|phi>|^2 K(E - E_j), K = the windowed kernel of a single level
+    c2 = np.abs(Vec.T @ phi) ** 2
+    nn_ = np.arange(-Nm, Nm + 1)
+    w = 0.5 * (1 + np.cos(np.pi * nn_ / (Nm + 1)))
+    K = lambda d: dtau / (2 * np.pi * HBAR) * np.sum(w * np.cos(np.outer(d, nn_) * dtau / HBAR), axis=1)
+    exact = np.array([np.sum(c2 * K(e - E)) for e in en])
+    assert relerr(ftm, exact) < 1e-11
+    # KPM (Jackson, energy-dependent width) and FTM (Hanning, uniform width) broaden differently, so
+    # they are compared where broadening drops out: the integrated DOS N(E) = int^E rho dE'
+    fine = np.linspace(-8.4, 8.4, 841)
+    de = fine[1] - fine[0]
+    n_ftm = np.cumsum(kgo.ftm_reconstruct(F, dtau, fine)) * de
+    n_kpm = np.cumsum(kgo.kpm_reconstruct(kgo.dos_moments(lat, 0.0, s, phi, 3 * Nm), 0.0, s, fine)) * de
+    assert abs(n_ftm[-1] - 1.0) < 1e-3 and abs(n_kpm[-1] - 1.0) < 1e-3
+    assert np.max(np.abs(n_kpm - n_ftm)) < 0.01
