@@ -46,17 +46,18 @@ UNIT = "Gsite-updates/s"
 # algorithmic bytes per site-update of the dominant kernel (fused recursion + moment dot,
 # general ELL, K = 3): 48 (T_m, T_{m-1}, T_{m+1}) + 16 (phi_L) + (12 idx + 24 hop + 8 onsite)/R
 # -- SURVEY.md 8(d), DESIGN.md "Roofline".
-def mom_bytes_per_update(R: int, kmax: int = 3) -> float:
-    return 48.0 + 16.0 + (kmax * 12.0 + 8.0) / R
+def mom_bytes_per_update(R: int, kmax: int = 3, phi_l_stream: bool = True) -> float:
+    return 48.0 + (16.0 if phi_l_stream else 0.0) + (kmax * 12.0 + 8.0) / R
 
 
 def site_updates(n: int, R: int, M: int, nt: int, n_p: int, doubling: bool = False) -> dict:
     """H~-applications one step really performs.  The oracle runs the literal
-    Alg. 5 (M-1 applications per moment set); the CUDA path gets two moments per application when
-    phi_L = phi_R (DOS, MSD: M/2 applications) and is credited only with those."""
+    Alg. 5 (M-1 applications per moment set); the CUDA path gets two moments per sweep from the
+    product identity: M/2 applications per set when phi_L = phi_R (DOS, MSD),
+    2 * (M/2) for VAC, whose sweep advances both phi_L and phi_R; it is credited only with those."""
     per_set = M // 2 if doubling else M - 1
     dos = per_set
-    vac = 1 + (nt + 1) * (1 + (M - 1)) + nt * 2 * (n_p - 1)
+    vac = 1 + (nt + 1) * (1 + (2 * (M // 2) if doubling else M - 1)) + nt * 2 * (n_p - 1)
     msd = (nt + 1) * per_set + nt * 2 * (n_p - 1)
     per_vec = {"dos": dos, "vac": vac, "msd": msd}
     return {k: v * n * R for k, v in per_vec.items()}
@@ -278,30 +279,33 @@ def run_b200(args, cfg):
     mu_avg = ctx.mean_over_ranks(mu_dos.mean(dim=0))
     mu0 = complex(mu_avg[0].item())
 
-    # dominant kernel: fused recursion + dot with distinct phi_L / phi_R (the VAC moment loop:
-    # 2 x 2999 of the step's ~9000 sweeps).  kg_moments(M) is M-2 such launches + 1 first-step
-    # launch of the same shape + 1 tiny reduction; average launch time = event time / (M-1).
-    phi_left = phi_dev.clone()
-    B.moments(h, phi_left, phi_dev, M, mu=mu_dos)
+    # dominant kernel (52 % of the step, profiles/): the VAC moment sweep kg_staged_kernel<2R,
+    # MODE_MOMX>, which advances the batch [V psi | chi] (2R columns) and accumulates the two cross
+    # inner products.  kg_vac(M, n_steps = 0) is M/2 - 1 such launches + 1 first-step launch of the
+    # same shape + velocity, column copy and reduction (< 0.3 % of the call): average launch time
+    # = event time / (M/2).  Algorithmic bytes per site-update (doubling row: no
+    # phi_L stream): 48 + 44/(2R); one launch makes n * 2R updates.
+    mu_v0 = torch.empty((R, 1, M), dtype=torch.complex128, device="cuda")
+    B.vac(h, phi_dev, M, 0, cfg.dt_fs, mu=mu_v0)
     reps = 3
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
     for _ in range(reps):
-        B.moments(h, phi_left, phi_dev, M, mu=mu_dos)
+        B.vac(h, phi_dev, M, 0, cfg.dt_fs, mu=mu_v0)
     e1.record(stream)
     torch.cuda.synchronize()
-    kern_us = e0.elapsed_time(e1) * 1e3 / (reps * (M - 1))
+    kern_us = e0.elapsed_time(e1) * 1e3 / (reps * (M // 2))
     peak, peak_src = peaks()
-    bytes_launch = mom_bytes_per_update(R, lat.kmax) * n * R
+    bytes_launch = mom_bytes_per_update(2 * R, lat.kmax, phi_l_stream=False) * n * 2 * R
     achieved = bytes_launch / (kern_us * 1e-6) / 1e9
-    traffic = ncu_traffic(f"{cfg.name}_mom_R{R}")
-    roofline = {"bound": "hbm", "kernel": f"kg_staged_kernel<R={R}, MODE_MOM> (fused T_m+1 = 2H~T_m - T_m-1 + <phi_L|T_m+1>; "
-                                         "TMA-staged streams, hopping dictionary, alternating sweep)",
+    traffic = ncu_traffic(f"{cfg.name}_momx_R{2 * R}")
+    roofline = {"bound": "hbm", "kernel": f"kg_staged_kernel<R={2 * R}, MODE_MOMX> (fused T_m+1 = 2H~T_m - T_m-1 on [phi_L | phi_R] "
+                                         "+ <T_m L|T_m+1 R>, <T_m+1 L|T_m+1 R>; TMA-staged streams, hopping dictionary, alternating sweep)",
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0,
                 "algorithmic_bytes_per_launch": bytes_launch, "us_per_launch": kern_us,
-                "gsu_per_s": n * R / (kern_us * 1e-6) / 1e9, "traffic": traffic}
+                "gsu_per_s": n * 2 * R / (kern_us * 1e-6) / 1e9, "traffic": traffic}
 
     if rank != 0:
         ctx.finalize()

@@ -165,6 +165,7 @@ static cudaError_t launch_step(kg_hamiltonian *h, int mode, bool first, int R, c
     case MODE_PAIR: return first ? launch_mf<MODE_PAIR, true>(h, R, a, grid, st) : launch_mf<MODE_PAIR, false>(h, R, a, grid, st);
     case MODE_VEL: return launch_mf<MODE_VEL, true>(h, R, a, grid, st);
     case MODE_MOM2: return first ? launch_mf<MODE_MOM2, true>(h, R, a, grid, st) : launch_mf<MODE_MOM2, false>(h, R, a, grid, st);
+    case MODE_MOMX: return first ? launch_mf<MODE_MOMX, true>(h, R, a, grid, st) : launch_mf<MODE_MOMX, false>(h, R, a, grid, st);
     }
     return cudaErrorInvalidValue;
 }
@@ -213,7 +214,9 @@ static cudaError_t staged_launch_m(const kg_hamiltonian *h, int R, const StagedA
     case 2: return staged_launch_rm<2, MODE>(h, a, p, st);
     case 4: return staged_launch_rm<4, MODE>(h, a, p, st);
     case 8: return staged_launch_rm<8, MODE>(h, a, p, st);
-    case 16: if (MODE == MODE_EVO) return staged_launch_rm<16, MODE_EVO>(h, a, p, st);
+    case 16:
+        if constexpr (MODE == MODE_EVO || MODE == MODE_MOMX) return staged_launch_rm<16, MODE>(h, a, p, st);
+        break;
     }
     return cudaErrorInvalidValue;
 }
@@ -226,6 +229,7 @@ static cudaError_t staged_launch(kg_hamiltonian *h, int mode, int R, const Stage
     case MODE_EVO: return staged_launch_m<MODE_EVO>(h, R, a, p, st);
     case MODE_PAIR: return staged_launch_m<MODE_PAIR>(h, R, a, p, st);
     case MODE_MOM2: return staged_launch_m<MODE_MOM2>(h, R, a, p, st);
+    case MODE_MOMX: return staged_launch_m<MODE_MOMX>(h, R, a, p, st);
     }
     return cudaErrorInvalidValue;
 }
@@ -234,7 +238,7 @@ static StagedPlan staged_plan(const kg_hamiltonian *h, int mode, int R)
 {
     StagedPlan p;
     memset(&p, 0, sizeof(p));
-    if (!h->staged || h->kmax != 3 || R > (mode == MODE_EVO ? 16 : 8)) return p;
+    if (!h->staged || h->kmax != 3 || R > ((mode == MODE_EVO || mode == MODE_MOMX) ? 16 : 8)) return p;
     const int te = sg_tile_e(mode);
     const size_t stage = (size_t)sg_stage_bytes(R, mode, h->has_onsite, h->ndict > 0);
     const size_t header = (size_t)sg_header_bytes(R);
@@ -588,15 +592,17 @@ extern "C" int kg_set_option(kg_hamiltonian *h, int option, int64_t value)
 // --------------------------------------------------------------------------------------
 
 // enqueue the M-1 fused recursion+dot kernels of Alg. 5 (a2+a3); partials [M][grid][R]
+// mode MODE_MOM: literal Alg. 5, R columns.  MODE_MOM2 (phi_L = phi_R) and MODE_MOMX (phiR is the
+// batch [phi_L | phi_R], R = total columns, partial rows R/2 wide): step m produces T_m and the
+// partials of moments 2m-1 and 2m, so the loop stops at m = M/2
+// (2 T_a T_b = T_{a+b} + T_{|a-b|}; kg_reduce_partials finishes it).
 static int enqueue_moment_steps(kg_hamiltonian *h, const c128 *phiL, int ldL, const c128 *phiR, int ldR,
                                 int R, int M, c128 *ta, c128 *tb, c128 *part, int grid,
-                                const StagedPlan &sp, bool dbl, cudaStream_t st)
+                                const StagedPlan &sp, int mode, cudaStream_t st)
 {
-    // dbl (phi_L = phi_R): step m produces T_m and the partials of moments 2m-1 and 2m, so the
-    // loop stops at m = M/2 (2 T_a T_b = T_{a+b} + T_{|a-b|}; kg_reduce_partials finishes it)
-    const int mode = dbl ? MODE_MOM2 : MODE_MOM;
+    const bool dbl = mode != MODE_MOM;
     const int m_end = dbl ? M / 2 + 1 : M;
-    const size_t prow = (size_t)grid * R;
+    const size_t prow = (size_t)grid * (mode == MODE_MOMX ? R / 2 : R);
     StagedArgs sa = staged_base_args(h, sp);
     sa.aux = phiL;
     StepArgs a = base_args(h);
@@ -634,12 +640,16 @@ static bool want_graph(const kg_hamiltonian *h, int64_t elems, cudaStream_t st)
 }
 
 // mu[r*mu_rstride + m] = <phiL_r | T_m(H~) | phiR_r>, m < M
+// cross = true: phiL == phiR is the batch [phi_L | phi_R] with R columns in total (MODE_MOMX);
+// mu gets R/2 rows.
 static int moments_device(kg_hamiltonian *h, const c128 *phiL, int ldL, const c128 *phiR, int ldR, int R,
-                          int M, c128 *mu, int64_t mu_rstride, cudaStream_t st)
+                          int M, c128 *mu, int64_t mu_rstride, cudaStream_t st, bool cross = false)
 {
     const int64_t elems = h->n * R;
-    const bool dbl = h->doubling && phiL == phiR && ldL == ldR;
-    const StagedPlan sp = staged_plan(h, dbl ? MODE_MOM2 : MODE_MOM, R);
+    const bool dbl = cross || (h->doubling && phiL == phiR && ldL == ldR);
+    const int mode = cross ? MODE_MOMX : dbl ? MODE_MOM2 : MODE_MOM;
+    const int PR = cross ? R / 2 : R;                        // columns of a partial row / rows of mu
+    const StagedPlan sp = staged_plan(h, mode, R);
     const int grid = sp.ok ? sp.grid : grid_for(h, elems);   // one partial row shape for both kernels
     void *ta, *tb, *part;
     int rc;
@@ -650,13 +660,13 @@ static int moments_device(kg_hamiltonian *h, const c128 *phiL, int ldL, const c1
         cudaGraphExec_t exec = nullptr;
         for (auto &g : h->graphs)
             if (g.phiL == phiL && g.phiR == phiR && g.ldL == ldL && g.ldR == ldR && g.R == R && g.M == M &&
-                g.grid == grid && g.threads == h->threads && g.dbl == (int)dbl)
+                g.grid == grid && g.threads == h->threads && g.dbl == mode)
                 exec = g.exec;
         if (!exec) {
             cudaGraph_t graph;
             CUDA_TRY(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
             const int64_t before = h->launches;
-            rc = enqueue_moment_steps(h, phiL, ldL, phiR, ldR, R, M, (c128 *)ta, (c128 *)tb, (c128 *)part, grid, sp, dbl, st);
+            rc = enqueue_moment_steps(h, phiL, ldL, phiR, ldR, R, M, (c128 *)ta, (c128 *)tb, (c128 *)part, grid, sp, mode, st);
             h->launches = before;
             cudaError_t e = cudaStreamEndCapture(st, &graph);
             if (rc) { if (e == cudaSuccess) cudaGraphDestroy(graph); return rc; }
@@ -665,16 +675,16 @@ static int moments_device(kg_hamiltonian *h, const c128 *phiL, int ldL, const c1
             cudaGraphDestroy(graph);
             if (e != cudaSuccess) return fail(KG_ECUDA, "graph instantiate: %s", cudaGetErrorString(e));
             if (h->graphs.size() >= 8) { cudaGraphExecDestroy(h->graphs.front().exec); h->graphs.erase(h->graphs.begin()); }
-            h->graphs.push_back(GraphEntry{phiL, phiR, ldL, ldR, R, M, grid, h->threads, (int)dbl, exec});
+            h->graphs.push_back(GraphEntry{phiL, phiR, ldL, ldR, R, M, grid, h->threads, mode, exec});
         }
         CUDA_TRY(cudaGraphLaunch(exec, st));
         h->launches += dbl ? M / 2 : M - 1;
     } else {
-        if ((rc = enqueue_moment_steps(h, phiL, ldL, phiR, ldR, R, M, (c128 *)ta, (c128 *)tb, (c128 *)part, grid, sp, dbl, st)))
+        if ((rc = enqueue_moment_steps(h, phiL, ldL, phiR, ldR, R, M, (c128 *)ta, (c128 *)tb, (c128 *)part, grid, sp, mode, st)))
             return rc;
     }
-    const int warps = M * R;
-    kg_reduce_partials<<<(warps * 32 + 255) / 256, 256, 0, st>>>((const c128 *)part, M, grid, R, mu, mu_rstride, dbl ? 1 : 0);
+    const int warps = M * PR;
+    kg_reduce_partials<<<(warps * 32 + 255) / 256, 256, 0, st>>>((const c128 *)part, M, grid, PR, mu, mu_rstride, dbl ? 1 : 0);
     h->launches++;
     CUDA_TRY(cudaGetLastError());
     return KG_OK;
@@ -904,7 +914,7 @@ extern "C" int kg_vac(kg_hamiltonian *h, const kg_c128 *phi, int R, int M, int n
     void *s0, *s1, *pl;
     OutStage o;
     if ((rc = stage_in(h, WS_IN0, phi, vbytes, st, &dphi)) || (rc = ws_get(h, WS_S0, 2 * vbytes, &s0)) ||
-        (rc = ws_get(h, WS_S1, 2 * vbytes, &s1)) || (rc = ws_get(h, WS_PHIL, vbytes, &pl)) ||
+        (rc = ws_get(h, WS_S1, 2 * vbytes, &s1)) || (rc = ws_get(h, WS_PHIL, 2 * vbytes, &pl)) ||
         (rc = stage_out(h, WS_MU, mu, (size_t)R * (n_steps + 1) * M * 16, &o)))
         return rc;
     // state S = [psi | chi] as one [n][2R] batch: psi_0 = phi, chi_0 = V phi  (Alg. 2)
@@ -915,8 +925,14 @@ extern "C" int kg_vac(kg_hamiltonian *h, const kg_c128 *phi, int R, int M, int n
     const int64_t rstride = (int64_t)(n_steps + 1) * M;
     for (int k = 0; k <= n_steps; ++k) {
         // phi_L = V psi_k, phi_R = chi_k
-        if ((rc = velocity_device(h, S, R2, (c128 *)pl, R, R, st)) ||
-            (rc = moments_device(h, (const c128 *)pl, R, S + R, R2, R, M, (c128 *)o.dev + (size_t)k * M, rstride, st)))
+        if (h->doubling) {
+            // cross-doubling: [V psi_k | chi_k] advanced as one 2R-wide batch, two moments per sweep
+            c128 *X0 = (c128 *)pl;
+            if ((rc = velocity_device(h, S, R2, X0, R2, R, st)) || (rc = copy_cols(h, S + R, R2, X0 + R, R2, R, st)) ||
+                (rc = moments_device(h, X0, R2, X0, R2, R2, M, (c128 *)o.dev + (size_t)k * M, rstride, st, true)))
+                return rc;
+        } else if ((rc = velocity_device(h, S, R2, (c128 *)pl, R, R, st)) ||
+                   (rc = moments_device(h, (const c128 *)pl, R, S + R, R2, R, M, (c128 *)o.dev + (size_t)k * M, rstride, st)))
             return rc;
         if (k == n_steps) break;
         // [psi | chi] <- U(-dt) [psi | chi]   (eqs 42-43), one 2R-wide batch

@@ -7,6 +7,10 @@
 //   MODE_MOM2  the same recursion for phi_L = phi_R = phi with the product identity
 //              2 T_a T_b = T_{a+b} + T_{|a-b|}: per-block partials of <T_m|T_{m+1}> (moment
 //              2m+1) and <T_{m+1}|T_{m+1}> (moment 2m+2) — two moments per sweep, no phi_L read
+//   MODE_MOMX  the same identity for phi_L != phi_R: the batch holds [phi_L | phi_R] as its two
+//              column halves, both are advanced by the recursion, and the partials are the CROSS
+//              products <T_m L|T_{m+1} R> (moment 2m+1) and <T_{m+1} L|T_{m+1} R> (moment 2m+2);
+//              one matrix read serves both chains and there is no separate phi_L stream (VAC)
 //   MODE_EVO   same recursion + out (+)= c_{m+1} T_{m+1}              (Alg. 6 l.5-6 P:383-385)
 //   MODE_PAIR  (a, d) pair recursion: a = T_m psi, d = T_m psix + [X,T_m] psi,
 //              d_{m+1} = alpha([X,H~] a_m + H~ d_m) - beta d_{m-1}    (eq 39, Alg. 7 l.7-8)
@@ -29,7 +33,7 @@
 
 typedef double2 c128;
 
-enum { MODE_MOM = 0, MODE_EVO = 1, MODE_PAIR = 2, MODE_VEL = 3, MODE_MOM2 = 4 };
+enum { MODE_MOM = 0, MODE_EVO = 1, MODE_PAIR = 2, MODE_VEL = 3, MODE_MOM2 = 4, MODE_MOMX = 5 };
 
 struct StepArgs {
     // matrix (device, library-owned)
@@ -118,7 +122,7 @@ __global__ void __launch_bounds__(256) kg_step_kernel(const StepArgs a)
         c128 acc = make_double2(0.0, 0.0);
         c128 dacc = make_double2(0.0, 0.0);
         c128 self = make_double2(0.0, 0.0), dself = make_double2(0.0, 0.0);
-        if (MODE != MODE_VEL && (ONS || FIRST || MODE == MODE_MOM2)) {
+        if (MODE != MODE_VEL && (ONS || FIRST || MODE == MODE_MOM2 || MODE == MODE_MOMX)) {
             self = ld_nc(a.cur + i * a.ld_cur + r);
             if (MODE == MODE_PAIR) dself = ld_nc(a.dcur + i * a.ld_dcur + r);
         }
@@ -172,6 +176,26 @@ __global__ void __launch_bounds__(256) kg_step_kernel(const StepArgs a)
             sum2.x = fma(t.x, t.x, fma(t.y, t.y, sum2.x));            // |T_{m+1}|^2
             if (FIRST) sum0.x = fma(self.x, self.x, fma(self.y, self.y, sum0.x));
         }
+        if (MODE == MODE_MOMX) {
+            // column r >= R/2 (right chain) pairs with column r - R/2 (left chain) of the same
+            // site, held by lane - R/2 of the same warp
+            constexpr int RH = R > 1 ? R / 2 : 1;
+            const unsigned mask = __activemask();
+            const int src = (threadIdx.x - RH) & 31;
+            c128 tl, sl;
+            tl.x = __shfl_sync(mask, t.x, src); tl.y = __shfl_sync(mask, t.y, src);
+            sl.x = __shfl_sync(mask, self.x, src); sl.y = __shfl_sync(mask, self.y, src);
+            if (r >= RH) {
+                sum.x = fma(sl.x, t.x, fma(sl.y, t.y, sum.x));        // conj(T_m L) * T_{m+1} R
+                sum.y = fma(sl.x, t.y, fma(-sl.y, t.x, sum.y));
+                sum2.x = fma(tl.x, t.x, fma(tl.y, t.y, sum2.x));      // conj(T_{m+1} L) * T_{m+1} R
+                sum2.y = fma(tl.x, t.y, fma(-tl.y, t.x, sum2.y));
+                if (FIRST) {
+                    sum0.x = fma(sl.x, self.x, fma(sl.y, self.y, sum0.x));
+                    sum0.y = fma(sl.x, self.y, fma(-sl.y, self.x, sum0.y));
+                }
+            }
+        }
         if (MODE == MODE_EVO || MODE == MODE_PAIR) {
             c128 o;
             if (FIRST) o = cmul(a.c0, self); else o = a.out[e];
@@ -194,17 +218,22 @@ __global__ void __launch_bounds__(256) kg_step_kernel(const StepArgs a)
         }
     }
 
-    if (MODE == MODE_MOM || MODE == MODE_MOM2) {
+    if (MODE == MODE_MOM || MODE == MODE_MOM2 || MODE == MODE_MOMX) {
         __shared__ c128 red[32 * R];
+        // MODE_MOMX: only the right-chain columns carry sums; partial rows are [grid][R/2]
+        constexpr int RH = (MODE == MODE_MOMX && R > 1) ? R / 2 : 0;
+        constexpr int PR = R - RH;
+        const bool writer = (int)threadIdx.x >= RH && (int)threadIdx.x < R;
+        const int64_t slot = (int64_t)blockIdx.x * PR + ((int)threadIdx.x - RH);
         c128 tot = block_reduce_per_r<R>(sum, red);
-        if (threadIdx.x < R) a.partial[(int64_t)blockIdx.x * R + threadIdx.x] = tot;
-        if (MODE == MODE_MOM2) {
+        if (writer) a.partial[slot] = tot;
+        if (MODE == MODE_MOM2 || MODE == MODE_MOMX) {
             c128 tot2 = block_reduce_per_r<R>(sum2, red);
-            if (threadIdx.x < R) a.partial2[(int64_t)blockIdx.x * R + threadIdx.x] = tot2;
+            if (writer) a.partial2[slot] = tot2;
         }
         if (FIRST) {
             c128 tot0 = block_reduce_per_r<R>(sum0, red);
-            if (threadIdx.x < R) a.partial0[(int64_t)blockIdx.x * R + threadIdx.x] = tot0;
+            if (writer) a.partial0[slot] = tot0;
         }
     }
 }

@@ -104,7 +104,7 @@ __device__ __forceinline__ void sg_bulk_g2s(uint32_t dst, const void *src, uint3
 // Tile size per mode: the pair recursion stages six vector streams, so its tile is half as long
 // to keep >= 2 stages x 3 CTAs per SM in shared memory.
 __host__ __device__ constexpr int sg_tile_e(int mode) { return mode == MODE_PAIR ? 256 : 512; }
-__host__ __device__ constexpr int sg_nvec(int mode) { return mode == MODE_PAIR ? 6 : mode == MODE_MOM2 ? 2 : 3; }
+__host__ __device__ constexpr int sg_nvec(int mode) { return mode == MODE_PAIR ? 6 : (mode == MODE_MOM2 || mode == MODE_MOMX) ? 2 : 3; }
 // bytes of one stage / of the header (host planning and device layout use the same formulas)
 __host__ __device__ constexpr int sg_stage_bytes(int R, int mode, bool ons, bool dict)
 {
@@ -138,6 +138,8 @@ struct SgLayout {
 // MODE_MOM   next = 2 H~ cur - prev ; partial += <phiL|next>            (Alg. 5 l.6-7)
 // MODE_MOM2  next = 2 H~ cur - prev ; partial += <cur|next>, partial2 += <next|next>
 //            (phi_L = phi_R: moments 2m+1 and 2m+2 from one sweep, see kg_kernels.cuh)
+// MODE_MOMX  the batch is [phi_L | phi_R] (R/2 columns each), both halves are advanced;
+//            partial += <cur_L|next_R>, partial2 += <next_L|next_R>, rows [grid][R/2]
 // MODE_EVO   next = 2 H~ cur - prev ; out += c1 next                     (Alg. 6 l.5-6)
 // MODE_PAIR  the same on the a-chain, and on the d-chain
 //            dnext = 2([X,H~] cur + H~ dcur) - dprev ; outd += c1 dnext  (eq 39, Alg. 7 l.7-8)
@@ -191,7 +193,7 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
                 sg_mbar_expect_tx(full, tx);
                 sg_bulk_g2s(sb + 0 * L::VEC, a.cur + e0, vbytes, full);
                 sg_bulk_g2s(sb + 1 * L::VEC, a.prev + e0, vbytes, full);
-                if (MODE != MODE_MOM2) sg_bulk_g2s(sb + 2 * L::VEC, a.aux + e0, vbytes, full);
+                if (sg_nvec(MODE) > 2) sg_bulk_g2s(sb + 2 * L::VEC, a.aux + e0, vbytes, full);
                 if (PAIR) {
                     sg_bulk_g2s(sb + 3 * L::VEC, a.dcur + e0, vbytes, full);
                     sg_bulk_g2s(sb + 4 * L::VEC, a.dprev + e0, vbytes, full);
@@ -286,6 +288,15 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
                         cfma_r(dacc, hk[q][k], dv[q][k]);               // H~ d_m
                     }
                 }
+                c128 tl = make_double2(0.0, 0.0);
+                if (MODE == MODE_MOMX) {
+                    // the left-chain partner (column r - R/2 of the same site) is lane - R/2;
+                    // every lane of the warp takes part (tail lanes carry unused values)
+                    const c128 p = prev_s[le];
+                    const int src = (tid - (R > 1 ? R / 2 : 1)) & 31;
+                    tl.x = __shfl_sync(0xffffffffu, fma(2.0, acc.x, -p.x), src);
+                    tl.y = __shfl_sync(0xffffffffu, fma(2.0, acc.y, -p.y), src);
+                }
                 if (le < ne) {
                     const c128 p = prev_s[le];
                     const c128 tt = make_double2(fma(2.0, acc.x, -p.x), fma(2.0, acc.y, -p.y));
@@ -294,6 +305,15 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
                         const c128 Lv = aux_s[le];
                         sum.x = fma(Lv.x, tt.x, fma(Lv.y, tt.y, sum.x));      // conj(L) * t
                         sum.y = fma(Lv.x, tt.y, fma(-Lv.y, tt.x, sum.y));
+                    } else if (MODE == MODE_MOMX) {
+                        constexpr int RH = R > 1 ? R / 2 : 1;
+                        if (r >= RH) {
+                            const c128 sl = self_s[le - RH];
+                            sum.x = fma(sl.x, tt.x, fma(sl.y, tt.y, sum.x));      // conj(T_m L) * T_{m+1} R
+                            sum.y = fma(sl.x, tt.y, fma(-sl.y, tt.x, sum.y));
+                            sum2.x = fma(tl.x, tt.x, fma(tl.y, tt.y, sum2.x));    // conj(T_{m+1} L) * T_{m+1} R
+                            sum2.y = fma(tl.x, tt.y, fma(-tl.y, tt.x, sum2.y));
+                        }
                     } else if (MODE == MODE_MOM2) {
                         const c128 sv = self_s[le];
                         sum.x = fma(sv.x, tt.x, fma(sv.y, tt.y, sum.x));      // conj(T_m) * T_{m+1}
@@ -316,13 +336,18 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
             if ((tid & 31) == 0) sg_mbar_arrive(empty0 + 8 * s);
         }
     }
-    if (MODE == MODE_MOM || MODE == MODE_MOM2) {
-        // block total per vector r (the producer warp adds zeros)
+    if (MODE == MODE_MOM || MODE == MODE_MOM2 || MODE == MODE_MOMX) {
+        // block total per column (the producer warp adds zeros); MODE_MOMX keeps the right-chain
+        // columns only: partial rows are [grid][R/2]
+        constexpr int RH = (MODE == MODE_MOMX && R > 1) ? R / 2 : 0;
+        constexpr int PR = R - RH;
+        const bool writer = tid >= RH && tid < R;
+        const int64_t slot = (int64_t)blockIdx.x * PR + (tid - RH);
         c128 tot = block_reduce_per_r<R>(sum, red);
-        if (tid < R) a.partial[(int64_t)blockIdx.x * R + tid] = tot;
-        if (MODE == MODE_MOM2) {
+        if (writer) a.partial[slot] = tot;
+        if (MODE != MODE_MOM) {
             c128 tot2 = block_reduce_per_r<R>(sum2, red);
-            if (tid < R) a.partial2[(int64_t)blockIdx.x * R + tid] = tot2;
+            if (writer) a.partial2[slot] = tot2;
         }
     }
 }

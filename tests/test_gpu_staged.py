@@ -212,3 +212,26 @@ def test_doubling_moments(B, kgo, M, R, staged):
     lit = host(B.dos_moments(h, d, M))
     assert h.launch_count - l0 == M                         # literal Alg. 5: M-1 sweeps + reduction
     assert relerr(mu, lit) <= 1e-13
+
+
+@pytest.mark.parametrize("R", [1, 2, 8])
+@pytest.mark.parametrize("staged", [0, 1])
+@pytest.mark.parametrize("M", [2, 3, 33, 48])
+def test_vac_cross_doubling(B, kgo, R, staged, M):
+    """VAC with phi_L != phi_R: [V psi | chi] advanced as one 2R-wide batch and
+    mu_{2m+1} = 2<T_m L|T_{m+1} R> - mu_1, mu_{2m+2} = 2<T_{m+1} L|T_{m+1} R> - mu_0 (MODE_MOMX)
+    against the oracle's literal Alg. 2 + Alg. 5, and against the literal GPU path."""
+    lat = sheet(40, 34, 90, True)           # 5350 sites: several tiles for every width
+    s = scale_for(lat)
+    olat = to_oracle_lattice(kgo, lat)
+    h = B.from_lattice(lat, lat.x, lat.period_x, 0.0, s)
+    h.set_option(B.KG_OPT_STAGED, staged)
+    phi = W.random_phase_vectors(lat.n, R, 12)
+    nt, dt = 2, 0.8
+    mu = host(B.vac(h, dev(phi), M, nt, dt))
+    for r in sorted({0, R - 1}):
+        want = kgo.vac(olat, olat.x, olat.period_x, 0.0, s, phi[:, r].copy(), M, nt, dt)
+        assert relerr(mu[r], want) <= TOL
+    h.set_option(B.KG_OPT_DOUBLING, 0)
+    lit = host(B.vac(h, dev(phi), M, nt, dt))
+    assert relerr(mu, lit) <= 1e-12
