@@ -242,12 +242,14 @@ static StagedPlan staged_plan(const kg_hamiltonian *h, int mode, int R)
     const int te = sg_tile_e(mode);
     const size_t stage = (size_t)sg_stage_bytes(R, mode, h->has_onsite, h->ndict > 0);
     const size_t header = (size_t)sg_header_bytes(R);
-    // auto: 3 CTAs per SM with a 2-deep ring measured best on config 4 (profiles/); fewer CTAs
-    // when a stage is too large for that (fp64 hoppings staged)
+    // auto: 3 CTAs per SM with a 2-deep ring measured best on configs 4 and 5 (profiles/): deeper
+    // rings only take shared memory away from the L1 that serves the out-of-tile gathers.  Fewer
+    // CTAs when a stage is too large for that (fp64 hoppings staged).
     int ctas = h->staged_ctas > 0 ? h->staged_ctas : 3, nst = 0;
     for (;; --ctas) {
         const size_t budget = (size_t)228 * 1024 / ctas - 1024;
         nst = h->stages > 0 ? h->stages : (int)((budget - header) / stage);
+        if (h->stages == 0 && nst > 2) nst = 2;
         if (nst >= 2 || h->staged_ctas > 0 || ctas == 1) break;
     }
     if (nst > SG_MAX_STAGES) nst = SG_MAX_STAGES;
