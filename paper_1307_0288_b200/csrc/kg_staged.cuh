@@ -44,7 +44,7 @@ struct StagedArgs {
     const double *hop;     // [3][ns]  H_ik / s              (used when !DICT)
     const double *xhop;    // [3][ns]  (X_i - X_m) H_ik / s  (MODE_PAIR)
     const double *onsite;  // [ns]     (H_ii - E0)/s         (used when ONS)
-    double dict[16];       // DICT: hopping value per id, dict[0] = 0
+    double dict[16];       // DICT: hopping value per id, dict[0] = 0 (read from the constant bank)
     int64_t n, ns;
     const c128 *cur;       // T_m      [n][R]
     const c128 *prev;      // T_{m-1}  [n][R]
@@ -151,7 +151,6 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
     constexpr bool PAIR = MODE == MODE_PAIR;
     extern __shared__ __align__(128) unsigned char sg_smem[];
     uint64_t *bars = reinterpret_cast<uint64_t *>(sg_smem);
-    double *dict_s = reinterpret_cast<double *>(sg_smem + L::OFF_DICT);
     c128 *red = reinterpret_cast<c128 *>(sg_smem + L::OFF_RED);
     unsigned char *stages = sg_smem + L::HEADER;
 
@@ -165,7 +164,6 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (DICT && tid < 16) dict_s[tid] = a.dict[tid];
     __syncthreads();
 
     const int64_t total = a.n * R;
@@ -251,7 +249,7 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
                     int64_t m;
                     if (DICT) {
                         m = w & SG_IDX_MASK;
-                        hk[q][k] = dict_s[(uint32_t)w >> 28];
+                        hk[q][k] = a.dict[(uint32_t)w >> 28];      // constant bank (LDC), not shared memory
                     } else {
                         m = w;
                         hk[q][k] = hop_s[k * CS + ls];
