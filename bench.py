@@ -199,7 +199,7 @@ def workload_config(cfg, args, n_ranks):
                         f"kg_vac + kg_msd with {args.time_steps} of the config's {cfg.n_steps} time steps",
             "sites": cfg.lattice.n, "R": cfg.R, "M": cfg.M, "time_steps": args.time_steps,
             "parallelism": f"replicas x{n_ranks} (independent random vectors, no data-path collective)",
-            "l2": "inputs larger than L2 (368 MB streamed per Chebyshev step vs 126 MB L2); no flush"}
+            "l2": "inputs larger than L2 (272-464 MB moved per Chebyshev sweep vs 126 MB L2); no flush"}
 
 
 # --------------------------------------------------------------------------------------

@@ -235,3 +235,52 @@ def test_vac_cross_doubling(B, kgo, R, staged, M):
     h.set_option(B.KG_OPT_DOUBLING, 0)
     lit = host(B.vac(h, dev(phi), M, nt, dt))
     assert relerr(mu, lit) <= 1e-12
+
+
+@pytest.mark.parametrize("R", [1, 8])
+def test_guard_bands_and_inputs_untouched(B, R):
+    """compute-sanitizer is closed on this pool, so out-of-bounds writes are looked for directly:
+    every caller-owned array sits between canary bands, sizes leave a ragged last tile, and after
+    each call the bands and the read-only inputs must be bit-identical to what they were."""
+    import torch
+    lat = sheet(33, 29, 61, True)                      # 3767 sites: ragged for both tile sizes
+    h = B.from_lattice(lat, lat.x, lat.period_x, 0.0, scale_for(lat))
+    n, G = lat.n, 4096
+    canary = complex(1.2345e300, -6.789e299)
+
+    def guarded(shape_rows, cols):
+        buf = torch.full((G + shape_rows * cols + G,), canary, dtype=torch.complex128, device="cuda")
+        return buf, buf[G:G + shape_rows * cols].view(shape_rows, cols)
+
+    def bands_ok(buf, rows, cols):
+        return bool((buf[:G] == canary).all()) and bool((buf[G + rows * cols:] == canary).all())
+
+    phi_np = W.random_phase_vectors(n, R, 2)
+    pbuf, phi = guarded(n, R)
+    phi.copy_(torch.from_numpy(phi_np))
+    keep = phi.clone()
+    M, nt = 37, 1
+    obuf, out = guarded(n, R)
+    B.evolve(h, phi, 0.8, out=out)
+    xbuf, psix = guarded(n, R)
+    psix.zero_()
+    qbuf, psi = guarded(n, R)
+    psi.copy_(phi)
+    B.evolve_x(h, psi, psix, 0.8)
+    vbuf, vout = guarded(n, R)
+    B.apply_velocity(h, phi, out=vout)
+    mbuf, mu = guarded(R, M)
+    B.dos_moments(h, phi, M, mu=mu)
+    cbuf, muv = guarded(R * (nt + 1), M)
+    B.vac(h, phi, M, nt, 0.8, mu=muv.view(R, nt + 1, M))
+    dbuf, mud = guarded(R * (nt + 1), M)
+    B.msd(h, phi, M, nt, 0.8, mu=mud.view(R, nt + 1, M))
+    fbuf, F = guarded(R, 7)
+    B.fourier_moments(h, phi, phi, 3, 0.3, F=F)
+    torch.cuda.synchronize()
+    assert torch.equal(phi, keep)                                     # inputs never modified
+    for buf, rows, cols in ((pbuf, n, R), (obuf, n, R), (xbuf, n, R), (qbuf, n, R), (vbuf, n, R),
+                            (mbuf, R, M), (cbuf, R * (nt + 1), M), (dbuf, R * (nt + 1), M), (fbuf, R, 7)):
+        assert bands_ok(buf, rows, cols)
+    for t in (out, psi, psix, vout, mu, muv, mud, F):                  # and every output was written
+        assert not bool((t == canary).any()) and bool(torch.isfinite(t.real).all())
