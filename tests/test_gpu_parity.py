@@ -403,3 +403,13 @@ def test_fourier_moments_and_ftm_reconstruct(B, kgo, R):
             assert relerr(f[r], kgo.ftm_reconstruct(Fh[r], dtau, en, window)) <= TOL
     f_host = B.ftm_reconstruct(Fh, dtau, en)
     assert relerr(f_host, host(B.ftm_reconstruct(Fd, dtau, dev(en)))) <= 1e-13
+
+
+def test_run_config_driver(B):
+    """The end-to-end driver (moments -> reconstruction -> transport) on config 1 in full."""
+    from paper_1307_0288_b200 import run_config
+    s = run_config.main(["--config", "1"])
+    assert abs(s["mu0"] - 1.0) < 1e-12
+    assert abs(s["dos_integral"] - 1.0) < 5e-3
+    assert abs(s["sigma_e2_over_e1_last"] - 0.5) < 0.05        # pristine sheet: ballistic, P:519
+    assert s["kernel_launches"] > 0
