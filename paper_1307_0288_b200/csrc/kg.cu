@@ -452,7 +452,7 @@ static int check_create_args(kg_hamiltonian **out, int64_t n, int64_t kmax, cons
     if (!out) return fail(KG_EINVAL, "out is NULL");
     *out = nullptr;
     if (!a || !b || !c || !x) return fail(KG_EINVAL, "NULL array argument");
-    if (n <= 0 || n >= (int64_t)1 << 31) return fail(KG_EINVAL, "n must be in [1, 2^31)");
+    if (n <= 0 || n >= ((int64_t)1 << 31) - 1024) return fail(KG_EINVAL, "n must be in [1, 2^31 - 1024)");
     if (kmax <= 0) return fail(KG_EINVAL, "kmax must be positive");
     if (kmax > 32) return fail(KG_EUNSUPPORTED, "kmax > 32 not supported");
     if (!(s > 0.0) || !std::isfinite(s) || !std::isfinite(e0) || !std::isfinite(period))

@@ -173,16 +173,17 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
     if (tid >= SG_CONSUMERS) {
         // ---------------- producer warp: one lane feeds the ring ----------------
         if (tid == SG_CONSUMERS) {
-            for (int j = 0; j < my_tiles; ++j) {
-                const int s = j % nst;
-                const uint32_t ph = (uint32_t)(j / nst) & 1u;
+            int s = 0;
+            uint32_t ph = 0;
+            for (int j = 0; j < my_tiles; ++j, ++s) {
+                if (s == nst) { s = 0; ph ^= 1u; }
                 int t = (int)blockIdx.x + j * (int)gridDim.x;
                 if (a.reverse) t = a.ntiles - 1 - t;
                 const int64_t site0 = (int64_t)t * CS, e0 = site0 * R;
                 const int64_t rem = total - e0;
                 const uint32_t vbytes = (uint32_t)(rem < TE ? rem : TE) * 16u;
                 const uint32_t full = full0 + 8 * s;
-                sg_mbar_wait(empty0 + 8 * s, ph ^ 1u);
+                while (!sg_mbar_try_wait(empty0 + 8 * s, ph ^ 1u)) __nanosleep(64);   // ring full: back off
                 const uint32_t sb = sg_smem_u32(stages + (size_t)s * L::STAGE);
                 uint32_t tx = (uint32_t)sg_nvec(MODE) * vbytes + 3u * CS * 4u;
                 if (ONS) tx += CS * 8u;
@@ -216,12 +217,14 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
     } else {
         // ---------------- consumers: gathers + arithmetic ----------------
         const int r = tid & (R - 1);
-        for (int j = 0; j < my_tiles; ++j) {
-            const int s = j % nst;
-            const uint32_t ph = (uint32_t)(j / nst) & 1u;
+        int s = 0;
+        uint32_t ph = 0;
+        for (int j = 0; j < my_tiles; ++j, ++s) {
+            if (s == nst) { s = 0; ph ^= 1u; }
             int t = (int)blockIdx.x + j * (int)gridDim.x;
             if (a.reverse) t = a.ntiles - 1 - t;
-            const int64_t site0 = (int64_t)t * CS, e0 = site0 * R;
+            const int32_t site0 = t * CS;                    // n < 2^31: site indices fit 32 bits
+            const int64_t e0 = (int64_t)site0 * R;
             const int64_t rem = total - e0;
             const int ne = (int)(rem < TE ? rem : TE);
             const unsigned char *sb = stages + (size_t)s * L::STAGE;
@@ -246,7 +249,7 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
 #pragma unroll
                 for (int k = 0; k < 3; ++k) {
                     const int32_t w = idx_s[k * CS + ls];
-                    int64_t m;
+                    int32_t m;
                     if (DICT) {
                         m = w & SG_IDX_MASK;
                         hk[q][k] = a.dict[(uint32_t)w >> 28];      // constant bank (LDC), not shared memory
@@ -254,13 +257,14 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
                         m = w;
                         hk[q][k] = hop_s[k * CS + ls];
                     }
-                    const int64_t d = m - site0;
-                    if ((uint64_t)d < (uint64_t)CS) {
-                        v[q][k] = self_s[(int)d * R + r];
-                        if (PAIR) dv[q][k] = dself_s[(int)d * R + r];
+                    const uint32_t d = (uint32_t)(m - site0);
+                    if (d < (uint32_t)CS) {
+                        v[q][k] = self_s[d * R + r];
+                        if (PAIR) dv[q][k] = dself_s[d * R + r];
                     } else {
-                        v[q][k] = ld_nc(a.cur + m * R + r);
-                        if (PAIR) dv[q][k] = ld_nc(a.dcur + m * R + r);
+                        const int64_t g = (int64_t)m * R + r;
+                        v[q][k] = ld_nc(a.cur + g);
+                        if (PAIR) dv[q][k] = ld_nc(a.dcur + g);
                     }
                 }
             }
