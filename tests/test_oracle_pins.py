@@ -571,3 +571,34 @@ def test_ftm_and_kpm_dos_agree(kgo):
     n_kpm = np.cumsum(kgo.kpm_reconstruct(kgo.dos_moments(lat, 0.0, s, phi, 3 * Nm), 0.0, s, fine)) * de
     assert abs(n_ftm[-1] - 1.0) < 1e-3 and abs(n_kpm[-1] - 1.0) < 1e-3
     assert np.max(np.abs(n_kpm - n_ftm)) < 0.01
+
+
+def test_open_boundary_length_saturates_at_sample_length(kgo):
+    """Fig. 3: with a non-periodic boundary along the transport direction the length
+    L(E,t) = 2 sqrt(DeltaX^2) (eq 50) is confined by the sample — "the maximum diffusion length ...
+    being the length of the sample" — while with periodic boundaries it keeps growing ballistically.
+    Pristine sheet 24 x 6 cells, L_x = 24 sqrt(3) a = 5.90 nm, site-localised start in the middle
+    so that no stochastic error enters."""
+    ncx, ncy = 24, 6
+    Lx = ncx * np.sqrt(3.0) * A
+    s, M, nt, dt = S_GRAPHENE, 48, 14, 4 * HBAR / 2.7
+    en = np.linspace(-2.0, 2.0, 9)
+    en = en[np.abs(en) > 0.4]
+    lengths = {}
+    for periodic in (False, True):
+        lat = kgo.honeycomb(ncx, ncy, periodic_x=periodic, periodic_y=True)
+        assert abs((lat.period_x if periodic else Lx) - Lx) < 1e-12
+        phi = np.zeros(lat.n, complex)
+        phi[4 * (3 * ncx + ncx // 2)] = 1.0
+        rho = kgo.kpm_reconstruct(kgo.dos_moments(lat, 0.0, s, phi, M), 0.0, s, en)
+        mu = kgo.msd(lat, lat.x, lat.period_x if periodic else 0.0, 0.0, s, phi, M, nt, dt)
+        fmsd = np.stack([kgo.kpm_reconstruct(mu[k], 0.0, s, en) for k in range(nt + 1)])
+        lengths[periodic] = kgo.transport(rho, None, fmsd, dt, 1.0)["length_nm"]
+    open_, pbc = lengths[False], lengths[True]
+    # early times: identical (the wave has not reached the edges yet)
+    assert np.max(np.abs(open_[1] - pbc[1])) < 1e-6 * np.max(pbc[1])
+    # late times: confined vs ballistic
+    assert np.max(open_) < 1.05 * Lx
+    assert np.max(open_[-4:]) > 0.6 * Lx
+    assert np.min(pbc[-1]) > 1.5 * Lx
+    assert np.all(np.diff(pbc.mean(axis=1)) > 0)
