@@ -4,6 +4,7 @@
 #include "kg.h"
 #include "kg_kernels.cuh"
 #include "kg_staged.cuh"
+#include "kg_staged_launch.h"
 
 #include <algorithm>
 #include <cmath>
@@ -183,53 +184,18 @@ static StepArgs base_args(const kg_hamiltonian *h)
 // ---- staged kernels (kg_staged.cuh): plan + dispatch ----
 struct StagedPlan { bool ok; int grid, nst, ntiles; size_t smem; };
 
-template <int R, int MODE, bool ONS, bool DICT>
-static cudaError_t staged_launch_t(const kg_hamiltonian *h, const StagedArgs &a, const StagedPlan &p, cudaStream_t st)
-{
-    static size_t configured[64] = {0};
-    const int dev = h->device & 63;
-    if (configured[dev] < p.smem) {
-        cudaError_t e = cudaFuncSetAttribute(kg_staged_kernel<R, MODE, ONS, DICT>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem);
-        if (e != cudaSuccess) return e;
-        configured[dev] = p.smem;
-    }
-    kg_staged_kernel<R, MODE, ONS, DICT><<<p.grid, SG_THREADS, p.smem, st>>>(a);
-    return cudaGetLastError();
-}
-
-template <int R, int MODE>
-static cudaError_t staged_launch_rm(const kg_hamiltonian *h, const StagedArgs &a, const StagedPlan &p, cudaStream_t st)
-{
-    const bool dict = h->ndict > 0;
-    if (h->has_onsite) return dict ? staged_launch_t<R, MODE, true, true>(h, a, p, st) : staged_launch_t<R, MODE, true, false>(h, a, p, st);
-    return dict ? staged_launch_t<R, MODE, false, true>(h, a, p, st) : staged_launch_t<R, MODE, false, false>(h, a, p, st);
-}
-
-template <int MODE>
-static cudaError_t staged_launch_m(const kg_hamiltonian *h, int R, const StagedArgs &a, const StagedPlan &p, cudaStream_t st)
-{
-    switch (R) {
-    case 1: return staged_launch_rm<1, MODE>(h, a, p, st);
-    case 2: return staged_launch_rm<2, MODE>(h, a, p, st);
-    case 4: return staged_launch_rm<4, MODE>(h, a, p, st);
-    case 8: return staged_launch_rm<8, MODE>(h, a, p, st);
-    case 16:
-        if constexpr (MODE == MODE_EVO || MODE == MODE_MOMX) return staged_launch_rm<16, MODE>(h, a, p, st);
-        break;
-    }
-    return cudaErrorInvalidValue;
-}
-
+// The staged kernels are compiled one row width K per translation unit (kg_staged_k<K>.cu) so
+// that the build can run them in parallel; kg_staged_launch.h declares their entry points.
 static cudaError_t staged_launch(kg_hamiltonian *h, int mode, int R, const StagedArgs &a, const StagedPlan &p, cudaStream_t st)
 {
     h->launches++;
-    switch (mode) {
-    case MODE_MOM: return staged_launch_m<MODE_MOM>(h, R, a, p, st);
-    case MODE_EVO: return staged_launch_m<MODE_EVO>(h, R, a, p, st);
-    case MODE_PAIR: return staged_launch_m<MODE_PAIR>(h, R, a, p, st);
-    case MODE_MOM2: return staged_launch_m<MODE_MOM2>(h, R, a, p, st);
-    case MODE_MOMX: return staged_launch_m<MODE_MOMX>(h, R, a, p, st);
+    StagedLaunch l;
+    l.grid = p.grid; l.smem = p.smem; l.device = h->device; l.has_onsite = h->has_onsite; l.dict = h->ndict > 0;
+    switch (h->kmax) {
+    case 2: return kg_staged_launch_k2(mode, R, a, l, st);
+    case 3: return kg_staged_launch_k3(mode, R, a, l, st);
+    case 4: return kg_staged_launch_k4(mode, R, a, l, st);
+    case 6: return kg_staged_launch_k6(mode, R, a, l, st);
     }
     return cudaErrorInvalidValue;
 }
@@ -238,9 +204,9 @@ static StagedPlan staged_plan(const kg_hamiltonian *h, int mode, int R)
 {
     StagedPlan p;
     memset(&p, 0, sizeof(p));
-    if (!h->staged || h->kmax != 3 || R > ((mode == MODE_EVO || mode == MODE_MOMX) ? 16 : 8)) return p;
+    if (!h->staged || !sg_k_supported(h->kmax) || R > ((mode == MODE_EVO || mode == MODE_MOMX) ? 16 : 8)) return p;
     const int te = sg_tile_e(mode);
-    const size_t stage = (size_t)sg_stage_bytes(R, mode, h->has_onsite, h->ndict > 0);
+    const size_t stage = (size_t)sg_stage_bytes(R, h->kmax, mode, h->has_onsite, h->ndict > 0);
     const size_t header = (size_t)sg_header_bytes(R);
     // auto: 3 CTAs per SM with a 2-deep ring measured best on configs 4 and 5 (profiles/): deeper
     // rings only take shared memory away from the L1 that serves the out-of-tile gathers.  Fewer
@@ -402,7 +368,7 @@ static int create_from_device_list(kg_hamiltonian **out, int64_t n, int kmax, co
     if (rc) return cleanup(rc);
     h->has_onsite = d_ons != nullptr || e0 != 0.0;
     // hopping dictionary for the staged kernel: <= 15 distinct non-zero values of H_ik/s
-    if (kmax == 3 && n <= (int64_t)SG_IDX_MASK + 1) {
+    if (sg_k_supported(kmax) && n <= (int64_t)SG_IDX_MASK + 1) {
         unsigned long long tab[16];
         for (int q = 0; q < 16; ++q) tab[q] = SG_DICT_EMPTY;
         tab[15] = 0;   // overflow flag lives in slot 15

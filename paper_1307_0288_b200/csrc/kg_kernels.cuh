@@ -1,110 +1,8 @@
-// kg_kernels.cuh — device kernels of libkg (sm_100a).
-//
-// One fused kernel family implements every step of the hot path:
-//
-//   MODE_MOM   T_{m+1} = alpha H~ T_m - beta T_{m-1}  (eq 38)  + per-block partial of
-//              <phi_L|T_{m+1}>  (Alg. 5 l.6-7 P:363-365; the paper's K3 and K5 in one pass)
-//   MODE_MOM2  the same recursion for phi_L = phi_R = phi with the product identity
-//              2 T_a T_b = T_{a+b} + T_{|a-b|}: per-block partials of <T_m|T_{m+1}> (moment
-//              2m+1) and <T_{m+1}|T_{m+1}> (moment 2m+2) — two moments per sweep, no phi_L read
-//   MODE_MOMX  the same identity for phi_L != phi_R: the batch holds [phi_L | phi_R] as its two
-//              column halves, both are advanced by the recursion, and the partials are the CROSS
-//              products <T_m L|T_{m+1} R> (moment 2m+1) and <T_{m+1} L|T_{m+1} R> (moment 2m+2);
-//              one matrix read serves both chains and there is no separate phi_L stream (VAC)
-//   MODE_EVO   same recursion + out (+)= c_{m+1} T_{m+1}              (Alg. 6 l.5-6 P:383-385)
-//   MODE_PAIR  (a, d) pair recursion: a = T_m psi, d = T_m psix + [X,T_m] psi,
-//              d_{m+1} = alpha([X,H~] a_m + H~ d_m) - beta d_{m-1}    (eq 39, Alg. 7 l.7-8)
-//              + both series accumulations                            (eq 44)
-//   MODE_VEL   out = V in = -(i s/hbar) [X,H~] in                     (eq 15)
-//
-// Layout: vectors [n][R] complex128 (double2), one THREAD PER ELEMENT (site i, vector r),
-// e = i*R + r, so the R lanes of a site read R consecutive 16-byte values: every own-element
-// access is a fully coalesced ld.global.v2.f64, every gather reads R*16 contiguous bytes, and
-// the matrix row (index, hopping, on-site) is fetched once per site and broadcast to R lanes.
-// The matrix is the paper's k-major neighbour list with row stride `ns` (n rounded up
-// to 32 so that each k-slab is 128-byte aligned).
-//
-// Determinism: a thread's elements are fixed by (grid, block), per-thread sums run in index
-// order, the warp/block reduction is a fixed tree, and kg_reduce_partials adds the per-block
-// partials in block order: moments are bitwise reproducible.
+// kg_kernels.cuh — device kernels of libkg (sm_100a) compiled into kg.cu: the one-thread-per-
+// element recursion kernel family, reductions, create-time kernels, post-processing.
+// (Shared types and helpers: kg_common.cuh; the TMA-staged kernels: kg_staged.cuh.)
 #pragma once
-#include <cuda_runtime.h>
-#include <stdint.h>
-
-typedef double2 c128;
-
-enum { MODE_MOM = 0, MODE_EVO = 1, MODE_PAIR = 2, MODE_VEL = 3, MODE_MOM2 = 4, MODE_MOMX = 5 };
-
-struct StepArgs {
-    // matrix (device, library-owned)
-    const int32_t *nl;    // [kmax][ns]
-    const double *hop;    // [kmax][ns]  H_ik / s
-    const double *xhop;   // [kmax][ns]  (X_i - X_m)_minimg H_ik / s   ([X,H~] weights)
-    const double *onsite; // [ns]        (H_ii - E0)/s
-    int64_t n;            // sites
-    int64_t ns;           // row stride of the k-major arrays
-    int kmax;
-    double alpha;         // 1 for the first step (T_1 = H~ T_0), 2 afterwards
-    // a-chain: element (i, r) of X at X[i*ld + r]
-    const c128 *cur;  int ld_cur;    // T_m      (gathered + own)
-    const c128 *prev; int ld_prev;   // T_{m-1}  (own element; unused when FIRST)
-    c128 *next;                      // T_{m+1}  (ld = R); may alias prev
-    // MODE_MOM
-    const c128 *phiL; int ld_L;
-    c128 *partial;                   // [grid][R] for moment m+1
-    c128 *partial0;                  // FIRST only: [grid][R] for moment 0
-    c128 *partial2;                  // MODE_MOM2: [grid][R] for moment 2m+2 (partial: 2m+1)
-    // MODE_EVO / MODE_PAIR: series accumulators (ld = R)
-    c128 *out;
-    c128 c0, c1;                     // FIRST: out = c0 cur + c1 next; else out += c1 next
-    // MODE_PAIR d-chain
-    const c128 *dcur; int ld_dcur;
-    const c128 *dprev; int ld_dprev;
-    c128 *dnext;
-    c128 *outd;
-    // MODE_VEL
-    c128 *vout; int ld_vout;
-    double vscale;                   // s / hbar
-};
-
-__device__ __forceinline__ c128 ld_nc(const c128 *p)
-{
-    return __ldg(reinterpret_cast<const double2 *>(p));
-}
-__device__ __forceinline__ c128 cmul(c128 a, c128 b)
-{
-    return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
-}
-__device__ __forceinline__ void cfma_r(c128 &acc, double h, c128 v)
-{
-    acc.x = fma(h, v.x, acc.x);
-    acc.y = fma(h, v.y, acc.y);
-}
-
-// Sum `v` over the lanes of a warp that share (lane % R), then over warps; thread tid < R of
-// the block ends up with the block total for vector r = tid.  Fixed tree => deterministic.
-template <int R>
-__device__ __forceinline__ c128 block_reduce_per_r(c128 v, c128 *smem /* [32][R] */)
-{
-#pragma unroll
-    for (int off = 16; off >= R; off >>= 1) {
-        v.x += __shfl_xor_sync(0xffffffffu, v.x, off);
-        v.y += __shfl_xor_sync(0xffffffffu, v.y, off);
-    }
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int nwarps = blockDim.x >> 5;
-    if (lane < R) smem[warp * R + lane] = v;
-    __syncthreads();
-    c128 tot = make_double2(0.0, 0.0);
-    if (threadIdx.x < R) {
-        for (int w = 0; w < nwarps; ++w) {
-            tot.x += smem[w * R + threadIdx.x].x;
-            tot.y += smem[w * R + threadIdx.x].y;
-        }
-    }
-    __syncthreads();
-    return tot;
-}
+#include "kg_common.cuh"
 
 // R = 16 or 32 lanes would leave nothing to shuffle for R = 32; supported R: 1, 2, 4, 8, 16.
 template <int R, int MODE, bool FIRST, bool ONS, int KMAX>
@@ -531,4 +429,47 @@ __global__ void kg_ftm_reconstruct_kernel(const c128 *__restrict__ F, int64_t ro
         sum = ns;
     }
     f[row * (int64_t)ne + j] = sum * dtau_over_hbar / (2.0 * 3.14159265358979323846);
+}
+
+// ---------------------------------------------------------------------------------------
+// create: hopping dictionary.  table[0..14] = bit patterns of the distinct non-zero values
+// of H_ik/s found so far (EMPTY = all ones, a NaN pattern no finite hopping has).
+// ---------------------------------------------------------------------------------------
+#define SG_DICT_EMPTY 0xFFFFFFFFFFFFFFFFull
+
+__global__ void kg_dict_collect(const double *__restrict__ hop, int64_t count,
+                                unsigned long long *table, unsigned int *overflow)
+{
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < count;
+         e += (int64_t)gridDim.x * blockDim.x) {
+        const double h = hop[e];
+        if (h == 0.0) continue;
+        const unsigned long long bits = (unsigned long long)__double_as_longlong(h);
+        bool found = false;
+        for (int sl = 0; sl < 15 && !found; ++sl) {
+            unsigned long long c = *((volatile unsigned long long *)table + sl);
+            if (c == SG_DICT_EMPTY) {
+                const unsigned long long old = atomicCAS(table + sl, SG_DICT_EMPTY, bits);
+                c = (old == SG_DICT_EMPTY) ? bits : old;
+            }
+            found = (c == bits);
+        }
+        if (!found) atomicOr(overflow, 1u);
+    }
+}
+
+// idx[e] = (id << 28) | nl[e], id = position of hop[e] in the sorted dictionary (0 for 0.0)
+__global__ void kg_dict_pack(const int32_t *__restrict__ nl, const double *__restrict__ hop,
+                             int64_t count, const double *__restrict__ dict, int ndict,
+                             int32_t *__restrict__ idx)
+{
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < count;
+         e += (int64_t)gridDim.x * blockDim.x) {
+        const double h = hop[e];
+        uint32_t id = 0;
+        if (h != 0.0)
+            for (int q = 1; q < ndict; ++q)
+                if (dict[q] == h) id = (uint32_t)q;
+        idx[e] = (int32_t)((id << 28) | (uint32_t)nl[e]);
+    }
 }

@@ -31,7 +31,7 @@
 // shape; per-thread sums run in a fixed order, the block tree is fixed, kg_reduce_partials
 // adds the per-CTA partials in CTA order.  Moments are bitwise reproducible run to run.
 #pragma once
-#include "kg_kernels.cuh"
+#include "kg_common.cuh"
 
 #define SG_TILE_E 512          // largest tile, elements (site, vector); row stride ns is a multiple
 #define SG_CONSUMERS 256       // consumer threads; + one producer warp
@@ -40,9 +40,9 @@
 #define SG_MAX_STAGES 8
 
 struct StagedArgs {
-    const int32_t *idx;    // [3][ns]  DICT: (id << 28) | NL_ik ; else NL_ik
-    const double *hop;     // [3][ns]  H_ik / s              (used when !DICT)
-    const double *xhop;    // [3][ns]  (X_i - X_m) H_ik / s  (MODE_PAIR)
+    const int32_t *idx;    // [K][ns]  DICT: (id << 28) | NL_ik ; else NL_ik
+    const double *hop;     // [K][ns]  H_ik / s              (used when !DICT)
+    const double *xhop;    // [K][ns]  (X_i - X_m) H_ik / s  (MODE_PAIR)
     const double *onsite;  // [ns]     (H_ii - E0)/s         (used when ONS)
     double dict[16];       // DICT: hopping value per id, dict[0] = 0 (read from the constant bank)
     int64_t n, ns;
@@ -106,11 +106,13 @@ __device__ __forceinline__ void sg_bulk_g2s(uint32_t dst, const void *src, uint3
 __host__ __device__ constexpr int sg_tile_e(int mode) { return mode == MODE_PAIR ? 256 : 512; }
 __host__ __device__ constexpr int sg_nvec(int mode) { return mode == MODE_PAIR ? 6 : (mode == MODE_MOM2 || mode == MODE_MOMX) ? 2 : 3; }
 // bytes of one stage / of the header (host planning and device layout use the same formulas)
-__host__ __device__ constexpr int sg_stage_bytes(int R, int mode, bool ons, bool dict)
+__host__ __device__ constexpr int sg_stage_bytes(int R, int K, int mode, bool ons, bool dict)
 {
-    return (sg_nvec(mode) * sg_tile_e(mode) * 16 + (sg_tile_e(mode) / R) * (12 + (ons ? 8 : 0) +
-            (mode == MODE_PAIR ? 24 : 0) + (dict ? 0 : 24)) + 127) / 128 * 128;
+    return (sg_nvec(mode) * sg_tile_e(mode) * 16 + (sg_tile_e(mode) / R) * (4 * K + (ons ? 8 : 0) +
+            (mode == MODE_PAIR ? 8 * K : 0) + (dict ? 0 : 8 * K)) + 127) / 128 * 128;
 }
+// row widths the staged kernels are compiled for (others run kg_step_kernel)
+__host__ __device__ constexpr bool sg_k_supported(int K) { return K == 2 || K == 3 || K == 4 || K == 6; }
 __host__ __device__ constexpr int sg_header_bytes(int R)
 {
     return (2 * SG_MAX_STAGES * 8 + 16 * 8 + 32 * R * 16 + 127) / 128 * 128;
@@ -119,20 +121,20 @@ __host__ __device__ constexpr int sg_header_bytes(int R)
 // byte offsets inside one stage.  Vector slots: 0 self (T_m of the tile), 1 prev (T_{m-1}),
 // 2 aux (phi_L for moments, the series accumulator for evolve / pair), 3-5 the same for the
 // d-chain of the pair recursion.
-template <int R, int MODE, bool ONS, bool DICT>
+template <int R, int K, int MODE, bool ONS, bool DICT>
 struct SgLayout {
     static constexpr int TE = sg_tile_e(MODE);
     static constexpr int CS = TE / R;                        // sites per tile
     static constexpr int VEC = TE * 16;
     static constexpr int OFF_IDX = sg_nvec(MODE) * VEC;
-    static constexpr int OFF_ONS = OFF_IDX + 3 * CS * 4;
+    static constexpr int OFF_ONS = OFF_IDX + K * CS * 4;
     static constexpr int OFF_XHOP = OFF_ONS + (ONS ? CS * 8 : 0);
-    static constexpr int OFF_HOP = OFF_XHOP + (MODE == MODE_PAIR ? 3 * CS * 8 : 0);
-    static constexpr int STAGE = sg_stage_bytes(R, MODE, ONS, DICT);
+    static constexpr int OFF_HOP = OFF_XHOP + (MODE == MODE_PAIR ? K * CS * 8 : 0);
+    static constexpr int STAGE = sg_stage_bytes(R, K, MODE, ONS, DICT);
     static constexpr int OFF_DICT = 2 * SG_MAX_STAGES * 8;
     static constexpr int OFF_RED = OFF_DICT + 16 * 8;
     static constexpr int HEADER = sg_header_bytes(R);
-    static_assert(OFF_HOP + (DICT ? 0 : 3 * CS * 8) <= STAGE, "stage layout");
+    static_assert(OFF_HOP + (DICT ? 0 : K * CS * 8) <= STAGE, "stage layout");
 };
 
 // MODE_MOM   next = 2 H~ cur - prev ; partial += <phiL|next>            (Alg. 5 l.6-7)
@@ -143,10 +145,10 @@ struct SgLayout {
 // MODE_EVO   next = 2 H~ cur - prev ; out += c1 next                     (Alg. 6 l.5-6)
 // MODE_PAIR  the same on the a-chain, and on the d-chain
 //            dnext = 2([X,H~] cur + H~ dcur) - dprev ; outd += c1 dnext  (eq 39, Alg. 7 l.7-8)
-template <int R, int MODE, bool ONS, bool DICT>
+template <int R, int K, int MODE, bool ONS, bool DICT>
 __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs a)
 {
-    typedef SgLayout<R, MODE, ONS, DICT> L;
+    typedef SgLayout<R, K, MODE, ONS, DICT> L;
     constexpr int CS = L::CS, TE = L::TE, EPT = TE / SG_CONSUMERS;
     constexpr bool PAIR = MODE == MODE_PAIR;
     extern __shared__ __align__(128) unsigned char sg_smem[];
@@ -185,10 +187,10 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
                 const uint32_t full = full0 + 8 * s;
                 while (!sg_mbar_try_wait(empty0 + 8 * s, ph ^ 1u)) __nanosleep(64);   // ring full: back off
                 const uint32_t sb = sg_smem_u32(stages + (size_t)s * L::STAGE);
-                uint32_t tx = (uint32_t)sg_nvec(MODE) * vbytes + 3u * CS * 4u;
+                uint32_t tx = (uint32_t)sg_nvec(MODE) * vbytes + (uint32_t)K * CS * 4u;
                 if (ONS) tx += CS * 8u;
-                if (PAIR) tx += 3u * CS * 8u;
-                if (!DICT) tx += 3u * CS * 8u;
+                if (PAIR) tx += (uint32_t)K * CS * 8u;
+                if (!DICT) tx += (uint32_t)K * CS * 8u;
                 sg_mbar_expect_tx(full, tx);
                 sg_bulk_g2s(sb + 0 * L::VEC, a.cur + e0, vbytes, full);
                 sg_bulk_g2s(sb + 1 * L::VEC, a.prev + e0, vbytes, full);
@@ -199,17 +201,17 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
                     sg_bulk_g2s(sb + 5 * L::VEC, a.daux + e0, vbytes, full);
                 }
 #pragma unroll
-                for (int k = 0; k < 3; ++k)
+                for (int k = 0; k < K; ++k)
                     sg_bulk_g2s(sb + L::OFF_IDX + k * CS * 4, a.idx + k * a.ns + site0, CS * 4u, full);
                 if (ONS) sg_bulk_g2s(sb + L::OFF_ONS, a.onsite + site0, CS * 8u, full);
                 if (PAIR) {
 #pragma unroll
-                    for (int k = 0; k < 3; ++k)
+                    for (int k = 0; k < K; ++k)
                         sg_bulk_g2s(sb + L::OFF_XHOP + k * CS * 8, a.xhop + k * a.ns + site0, CS * 8u, full);
                 }
                 if (!DICT) {
 #pragma unroll
-                    for (int k = 0; k < 3; ++k)
+                    for (int k = 0; k < K; ++k)
                         sg_bulk_g2s(sb + L::OFF_HOP + k * CS * 8, a.hop + k * a.ns + site0, CS * 8u, full);
                 }
             }
@@ -240,14 +242,14 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
             const double *hop_s = reinterpret_cast<const double *>(sb + L::OFF_HOP);
             sg_mbar_wait(full0 + 8 * s, ph);
 
-            c128 v[EPT][3], dv[PAIR ? EPT : 1][3];
-            double hk[EPT][3];
+            c128 v[EPT][K], dv[PAIR ? EPT : 1][K];
+            double hk[EPT][K];
 #pragma unroll
             for (int q = 0; q < EPT; ++q) {
                 const int le = tid + q * SG_CONSUMERS;
                 const int ls = le / R;
 #pragma unroll
-                for (int k = 0; k < 3; ++k) {
+                for (int k = 0; k < K; ++k) {
                     const int32_t w = idx_s[k * CS + ls];
                     int32_t m;
                     if (DICT) {
@@ -283,7 +285,7 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
                     }
                 }
 #pragma unroll
-                for (int k = 0; k < 3; ++k) {
+                for (int k = 0; k < K; ++k) {
                     cfma_r(acc, hk[q][k], v[q][k]);
                     if (PAIR) {
                         cfma_r(dacc, xhop_s[k * CS + ls], v[q][k]);     // [X,H~] a_m
@@ -354,45 +356,3 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
     }
 }
 
-// ---------------------------------------------------------------------------------------
-// create: hopping dictionary.  table[0..14] = bit patterns of the distinct non-zero values
-// of H_ik/s found so far (EMPTY = all ones, a NaN pattern no finite hopping has).
-// ---------------------------------------------------------------------------------------
-#define SG_DICT_EMPTY 0xFFFFFFFFFFFFFFFFull
-
-__global__ void kg_dict_collect(const double *__restrict__ hop, int64_t count,
-                                unsigned long long *table, unsigned int *overflow)
-{
-    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < count;
-         e += (int64_t)gridDim.x * blockDim.x) {
-        const double h = hop[e];
-        if (h == 0.0) continue;
-        const unsigned long long bits = (unsigned long long)__double_as_longlong(h);
-        bool found = false;
-        for (int sl = 0; sl < 15 && !found; ++sl) {
-            unsigned long long c = *((volatile unsigned long long *)table + sl);
-            if (c == SG_DICT_EMPTY) {
-                const unsigned long long old = atomicCAS(table + sl, SG_DICT_EMPTY, bits);
-                c = (old == SG_DICT_EMPTY) ? bits : old;
-            }
-            found = (c == bits);
-        }
-        if (!found) atomicOr(overflow, 1u);
-    }
-}
-
-// idx[e] = (id << 28) | nl[e], id = position of hop[e] in the sorted dictionary (0 for 0.0)
-__global__ void kg_dict_pack(const int32_t *__restrict__ nl, const double *__restrict__ hop,
-                             int64_t count, const double *__restrict__ dict, int ndict,
-                             int32_t *__restrict__ idx)
-{
-    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < count;
-         e += (int64_t)gridDim.x * blockDim.x) {
-        const double h = hop[e];
-        uint32_t id = 0;
-        if (h != 0.0)
-            for (int q = 1; q < ndict; ++q)
-                if (dict[q] == h) id = (uint32_t)q;
-        idx[e] = (int32_t)((id << 28) | (uint32_t)nl[e]);
-    }
-}

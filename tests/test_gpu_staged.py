@@ -284,3 +284,57 @@ def test_guard_bands_and_inputs_untouched(B, R):
         assert bands_ok(buf, rows, cols)
     for t in (out, psi, psix, vout, mu, muv, mud, F):                  # and every output was written
         assert not bool((t == canary).any()) and bool(torch.isfinite(t.real).all())
+
+
+def grid_lattice(shape, t=-1.0, a=0.3, seed=4, onsite_w=0.0):
+    """Simple hyper-cubic tight-binding lattice (chain / square / cubic), periodic in every
+    direction: kmax = 2 * dim neighbours per site in the paper's k-major list; x = first axis."""
+    dims = tuple(shape)
+    n = int(np.prod(dims))
+    coords = np.stack(np.unravel_index(np.arange(n), dims), axis=0)
+    nbrs = []
+    for ax in range(len(dims)):
+        for step in (+1, -1):
+            c = coords.copy()
+            c[ax] = (c[ax] + step) % dims[ax]
+            nbrs.append(np.ravel_multi_index(tuple(c), dims))
+    kmax = len(nbrs)
+    nl = np.concatenate(nbrs).astype(np.int32)
+    hop = np.full(kmax * n, t)
+    ons = None
+    if onsite_w:
+        ons = onsite_w * (np.random.default_rng(seed).random(n) - 0.5)
+    lat = W.Lattice(n, kmax, np.full(n, kmax, np.int32), nl, hop, ons, coords[0] * a,
+                    np.zeros(n), dims[0] * a, 0.0)
+    return lat
+
+
+@pytest.mark.parametrize("shape", [(5000,), (90, 70), (22, 18, 16)])
+@pytest.mark.parametrize("R", [1, 4])
+def test_staged_other_row_widths(B, kgo, shape, R):
+    """The staged kernels for K = 2, 4, 6 (chain, square, cubic Anderson models): moments with
+    distinct and identical vectors, VAC, MSD, evolve against the oracle, and against the
+    one-thread-per-element kernels."""
+    lat = grid_lattice(shape, onsite_w=1.0)
+    s = (lat.kmax * 1.0 + 0.5) * 1.05
+    olat = to_oracle_lattice(kgo, lat)
+    h = B.from_lattice(lat, lat.x, lat.period_x, 0.0, s)
+    phi = W.random_phase_vectors(lat.n, R, 9)
+    rng = np.random.default_rng(3)
+    L = rng.normal(size=(lat.n, R)) + 1j * rng.normal(size=(lat.n, R))
+    M, nt, dt = 30, 1, 0.9
+    got = {"mom": host(B.moments(h, dev(L), dev(phi), M)), "dos": host(B.dos_moments(h, dev(phi), M)),
+           "vac": host(B.vac(h, dev(phi), M, nt, dt)), "msd": host(B.msd(h, dev(phi), M, nt, dt)),
+           "evo": host(B.evolve(h, dev(phi), dt))}
+    r = R - 1
+    v = phi[:, r].copy()
+    assert relerr(got["mom"][r], kgo.moments(olat, 0.0, s, L[:, r].copy(), v, M)) <= TOL
+    assert relerr(got["dos"][r], kgo.dos_moments(olat, 0.0, s, v, M)) <= TOL
+    assert relerr(got["vac"][r], kgo.vac(olat, olat.x, olat.period_x, 0.0, s, v, M, nt, dt)) <= TOL
+    assert relerr(got["msd"][r], kgo.msd(olat, olat.x, olat.period_x, 0.0, s, v, M, nt, dt)) <= TOL
+    assert relerr(got["evo"][:, r], kgo.evolve(olat, 0.0, s, v, dt)) <= 1e-12
+    l0 = h.launch_count
+    h.set_option(B.KG_OPT_STAGED, 0)
+    assert relerr(host(B.vac(h, dev(phi), M, nt, dt)), got["vac"]) <= 1e-12
+    assert relerr(host(B.msd(h, dev(phi), M, nt, dt)), got["msd"]) <= 1e-12
+    assert h.launch_count > l0
