@@ -53,7 +53,11 @@ def main(argv=None):
     phi = torch.from_numpy(W.random_phase_vectors(n, R, cfg.seed)).cuda()
     energies = torch.from_numpy(W.energy_grid(cfg.n_energies)).cuda()
     t_setup = time.perf_counter() - t0
-    stream = torch.cuda.current_stream()
+    # a side stream: the library replays launch-bound moment loops as CUDA graphs, which the
+    # legacy default stream cannot capture
+    prev_stream = torch.cuda.current_stream()
+    stream = torch.cuda.Stream()
+    torch.cuda.set_stream(stream)
 
     def timed(fn):
         torch.cuda.synchronize()
@@ -94,6 +98,7 @@ def main(argv=None):
         return out
 
     pp, timing["post_s"], _ = timed(post)
+    torch.cuda.set_stream(prev_stream)
     host = {k: v.cpu().numpy() for k, v in {**res, **pp}.items() if v is not None}
     en = energies.cpu().numpy()
 
