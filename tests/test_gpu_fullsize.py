@@ -93,3 +93,24 @@ def test_config5_batched_prefix_parity(B, kgo):
         v = phi[:, r].copy()
         assert relerr(dos[r], kgo.dos_moments(olat, cfg.e0, cfg.scale, v, Mp)) <= TOL
         assert relerr(msd[r], kgo.msd(olat, cfg.xcoord, cfg.period, cfg.e0, cfg.scale, v, 4, 1, cfg.dt_fs)) <= TOL
+
+
+def test_full_recursion_depth_M3000(B, kgo):
+    """Rounding-error growth over the FULL recursion depth of configs 4-5 (M = 3000) on a lattice the
+    oracle can finish (160 x 160 cells = 102 400 sites, Anderson W = |t|, config 4's scale): all three
+    moment kernels — literal Alg. 5 (phi_L != phi_R), doubling (DOS) and cross-doubling (VAC, t = 0) —
+    against the oracle's literal recursion, every one of the 3000 moments, tolerance 1e-10."""
+    lat = W.honeycomb(160, 160)
+    lat.onsite = W.anderson(lat.n, 2.7, 2)
+    s = (3 * 2.7 + 1.35) * 1.05
+    olat = to_oracle_lattice(kgo, lat)
+    h = B.from_lattice(lat, lat.x, lat.period_x, 0.0, s)
+    M = 3000
+    phi = W.random_phase_vectors(lat.n, 2, 7)
+    a, b = phi[:, 0].copy(), phi[:, 1].copy()
+    dos = host(B.dos_moments(h, dev(a), M))[0]
+    assert relerr(dos, kgo.dos_moments(olat, 0.0, s, a, M)) <= TOL
+    mom = host(B.moments(h, dev(b), dev(a), M))[0]
+    assert relerr(mom, kgo.moments(olat, 0.0, s, b, a, M)) <= TOL
+    vac = host(B.vac(h, dev(a), M, 0, 1.0))[0]
+    assert relerr(vac, kgo.vac(olat, olat.x, olat.period_x, 0.0, s, a, M, 0, 1.0)) <= TOL
