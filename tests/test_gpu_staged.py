@@ -338,3 +338,15 @@ def test_staged_other_row_widths(B, kgo, shape, R):
     assert relerr(host(B.vac(h, dev(phi), M, nt, dt)), got["vac"]) <= 1e-12
     assert relerr(host(B.msd(h, dev(phi), M, nt, dt)), got["msd"]) <= 1e-12
     assert h.launch_count > l0
+
+
+@pytest.mark.parametrize("R", [1, 8])
+def test_vac_msd_bitwise_reproducible(B, R):
+    """No atomics anywhere on the path: repeated kg_vac / kg_msd calls (cross-doubling shuffles,
+    per-CTA partials, fixed-order final sum) give identical bits."""
+    lat = sheet(70, 60, 200, True)          # 16 600 sites
+    h = B.from_lattice(lat, lat.x, lat.period_x, 0.0, scale_for(lat))
+    phi = dev(W.random_phase_vectors(lat.n, R, 4))
+    a = host(B.vac(h, phi, 50, 2, 0.8)); b = host(B.vac(h, phi, 50, 2, 0.8))
+    c = host(B.msd(h, phi, 50, 2, 0.8)); d = host(B.msd(h, phi, 50, 2, 0.8))
+    assert a.tobytes() == b.tobytes() and c.tobytes() == d.tobytes()
