@@ -66,7 +66,7 @@ struct kg_hamiltonian {
     double *hop, *xhop, *onsite;
     double dict[16];          // hopping dictionary, dict[0] = 0
     int ndict;                // entries in use (0: hoppings do not fit a dictionary)
-    int staged, stages, staged_ctas, alternate, doubling;   // options of the staged kernel
+    int staged, stages, staged_ctas, alternate, doubling, clenshaw;   // options of the staged kernel
     void *ws[WS_COUNT];
     size_t ws_bytes[WS_COUNT];
     size_t matrix_bytes;
@@ -204,7 +204,7 @@ static StagedPlan staged_plan(const kg_hamiltonian *h, int mode, int R)
 {
     StagedPlan p;
     memset(&p, 0, sizeof(p));
-    if (!h->staged || !sg_k_supported(h->kmax) || R > ((mode == MODE_EVO || mode == MODE_MOMX) ? 16 : 8)) return p;
+    if (!h->staged || !sg_k_supported(h->kmax) || R > ((mode == MODE_EVO || mode == MODE_MOMX || mode == MODE_CLEN) ? 16 : 8)) return p;
     const int te = sg_tile_e(mode);
     const size_t stage = (size_t)sg_stage_bytes(R, h->kmax, mode, h->has_onsite, h->ndict > 0);
     const size_t header = (size_t)sg_header_bytes(R);
@@ -326,7 +326,7 @@ static int create_from_device_list(kg_hamiltonian **out, int64_t n, int kmax, co
     h->n = n; h->ns = (n + SG_TILE_E - 1) / SG_TILE_E * SG_TILE_E; h->kmax = kmax;
     h->s = s; h->e0 = e0; h->period = period;
     h->nl = h->nlp = nullptr; h->hop = h->xhop = h->onsite = nullptr;
-    h->ndict = 0; h->staged = 1; h->stages = 0; h->staged_ctas = 0; h->alternate = 1; h->doubling = 1;
+    h->ndict = 0; h->staged = 1; h->stages = 0; h->staged_ctas = 0; h->alternate = 1; h->doubling = 1; h->clenshaw = 1;
     memset(h->dict, 0, sizeof(h->dict));
     memset(h->ws, 0, sizeof(h->ws));
     memset(h->ws_bytes, 0, sizeof(h->ws_bytes));
@@ -545,6 +545,7 @@ extern "C" int kg_set_option(kg_hamiltonian *h, int option, int64_t value)
         h->staged_ctas = (int)value; break;
     case KG_OPT_ALTERNATE: h->alternate = value != 0; break;
     case KG_OPT_DOUBLING: h->doubling = value != 0; break;
+    case KG_OPT_CLENSHAW: h->clenshaw = value != 0; break;
     case KG_OPT_DICT:
         if (value != 0) return fail(KG_EINVAL, "the dictionary can only be switched off");
         h->ndict = 0; break;
@@ -673,6 +674,32 @@ static int evolve_device(kg_hamiltonian *h, const c128 *in, int ld_in, c128 *out
     std::vector<c128> c;
     series_coefficients(h, dt_fs, eps, c);
     const int np = (int)c.size();
+    const StagedPlan cp = staged_plan(h, MODE_CLEN, R);
+    if (h->clenshaw && cp.ok && ld_in == R && np >= 4) {
+        // Clenshaw's backward recurrence for sum_m c_m T_m(H~) phi (same series as Alg. 6, eq 36):
+        //   b_m = c_m phi + 2 H~ b_{m+1} - b_{m+2}  (b_np = b_{np+1} = 0),  U phi = c_0 phi + H~ b_1 - b_2.
+        // np - 1 staged sweeps, no accumulator stream.  The first two sweeps fold b_{np-1} = c_{np-1} phi
+        // into their coefficients so that it is never written.
+        StagedArgs ca = staged_base_args(h, cp);
+        ca.aux = in;
+        c128 *buf[2] = {(c128 *)ta, (c128 *)tb};
+        const c128 one = make_double2(1.0, 0.0);
+        for (int m = np - 2, k = 0; m >= 0; --m, ++k) {
+            ca.alpha = m == 0 ? 1.0 : 2.0;
+            ca.next = m == 0 ? out : buf[k & 1];
+            if (k == 0) {            // b_{np-2} = c_{np-2} phi + 2 c_{np-1} H~ phi
+                ca.cur = in; ca.prev = in; ca.c1 = c[m]; ca.cpre = c[np - 1]; ca.use_prev = 0;
+            } else if (k == 1) {     // b_{np-3} = (c_{np-3} - c_{np-1}) phi + 2 H~ b_{np-2}
+                ca.cur = buf[0]; ca.prev = buf[0]; ca.cpre = one; ca.use_prev = 0;
+                ca.c1 = make_double2(c[m].x - c[np - 1].x, c[m].y - c[np - 1].y);
+            } else {
+                ca.cur = buf[(k - 1) & 1]; ca.prev = buf[k & 1]; ca.c1 = c[m]; ca.cpre = one; ca.use_prev = 1;
+            }
+            ca.reverse = h->alternate ? (k & 1) : 0;
+            CUDA_TRY(staged_launch(h, MODE_CLEN, R, ca, cp, st));
+        }
+        return KG_OK;
+    }
     StepArgs a = base_args(h);
     a.out = out;
     a.alpha = 1.0;

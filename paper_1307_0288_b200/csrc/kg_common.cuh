@@ -13,6 +13,8 @@
 //              products <T_m L|T_{m+1} R> (moment 2m+1) and <T_{m+1} L|T_{m+1} R> (moment 2m+2);
 //              one matrix read serves both chains and there is no separate phi_L stream (VAC)
 //   MODE_EVO   same recursion + out (+)= c_{m+1} T_{m+1}              (Alg. 6 l.5-6 P:383-385)
+//   MODE_CLEN  (staged kernel only) the same series summed by Clenshaw's backward recurrence
+//              b_m = c_m phi + 2 H~ b_{m+1} - b_{m+2}: no accumulator stream
 //   MODE_PAIR  (a, d) pair recursion: a = T_m psi, d = T_m psix + [X,T_m] psi,
 //              d_{m+1} = alpha([X,H~] a_m + H~ d_m) - beta d_{m-1}    (eq 39, Alg. 7 l.7-8)
 //              + both series accumulations                            (eq 44)
@@ -34,7 +36,7 @@
 
 typedef double2 c128;
 
-enum { MODE_MOM = 0, MODE_EVO = 1, MODE_PAIR = 2, MODE_VEL = 3, MODE_MOM2 = 4, MODE_MOMX = 5 };
+enum { MODE_MOM = 0, MODE_EVO = 1, MODE_PAIR = 2, MODE_VEL = 3, MODE_MOM2 = 4, MODE_MOMX = 5, MODE_CLEN = 6 };
 
 struct StepArgs {
     // matrix (device, library-owned)

@@ -54,6 +54,9 @@ struct StagedArgs {
     c128 *partial2;        // MODE_MOM2: <T_{m+1}|T_{m+1}> (moment 2m+2)
     c128 *out;             // MODE_EVO / MODE_PAIR: out += c1 T_{m+1}
     c128 c1;
+    c128 cpre;             // MODE_CLEN: next = c1 aux + cpre (alpha H~ cur) - (use_prev ? prev : 0)
+    double alpha;
+    int use_prev;
     const c128 *dcur, *dprev, *daux;   // MODE_PAIR d-chain (daux = outd, read side)
     c128 *dnext, *outd;
     int ntiles;
@@ -143,6 +146,9 @@ struct SgLayout {
 // MODE_MOMX  the batch is [phi_L | phi_R] (R/2 columns each), both halves are advanced;
 //            partial += <cur_L|next_R>, partial2 += <next_L|next_R>, rows [grid][R/2]
 // MODE_EVO   next = 2 H~ cur - prev ; out += c1 next                     (Alg. 6 l.5-6)
+// MODE_CLEN  next = c1 phi + cpre (alpha H~ cur) - prev : Clenshaw's backward recurrence for the
+//            series of eq 36, b_m = c_m phi + 2 H~ b_{m+1} - b_{m+2}, U phi = c_0 phi + H~ b_1 - b_2
+//            (aux = phi; three read streams and one write instead of evolve's three and two)
 // MODE_PAIR  the same on the a-chain, and on the d-chain
 //            dnext = 2([X,H~] cur + H~ dcur) - dprev ; outd += c1 dnext  (eq 39, Alg. 7 l.7-8)
 template <int R, int K, int MODE, bool ONS, bool DICT>
@@ -303,9 +309,18 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
                 }
                 if (le < ne) {
                     const c128 p = prev_s[le];
-                    const c128 tt = make_double2(fma(2.0, acc.x, -p.x), fma(2.0, acc.y, -p.y));
+                    c128 tt;
+                    if (MODE == MODE_CLEN) {
+                        const c128 g = cmul(a.cpre, make_double2(a.alpha * acc.x, a.alpha * acc.y));
+                        const c128 ca = cmul(a.c1, aux_s[le]);
+                        tt = make_double2(ca.x + g.x, ca.y + g.y);
+                        if (a.use_prev) { tt.x -= p.x; tt.y -= p.y; }
+                    } else {
+                        tt = make_double2(fma(2.0, acc.x, -p.x), fma(2.0, acc.y, -p.y));
+                    }
                     a.next[e0 + le] = tt;
-                    if (MODE == MODE_MOM) {
+                    if (MODE == MODE_CLEN) {
+                    } else if (MODE == MODE_MOM) {
                         const c128 Lv = aux_s[le];
                         sum.x = fma(Lv.x, tt.x, fma(Lv.y, tt.y, sum.x));      // conj(L) * t
                         sum.y = fma(Lv.x, tt.y, fma(-Lv.y, tt.x, sum.y));

@@ -40,7 +40,7 @@ cudaError_t launch_m(int R, const StagedArgs &a, const StagedLaunch &l, cudaStre
     case 4: return launch_rm<4, K, MODE>(a, l, st);
     case 8: return launch_rm<8, K, MODE>(a, l, st);
     case 16:
-        if constexpr (MODE == MODE_EVO || MODE == MODE_MOMX) return launch_rm<16, K, MODE>(a, l, st);
+        if constexpr (MODE == MODE_EVO || MODE == MODE_MOMX || MODE == MODE_CLEN) return launch_rm<16, K, MODE>(a, l, st);
         break;
     }
     return cudaErrorInvalidValue;
@@ -55,6 +55,7 @@ cudaError_t launch_k(int mode, int R, const StagedArgs &a, const StagedLaunch &l
     case MODE_PAIR: return launch_m<K, MODE_PAIR>(R, a, l, st);
     case MODE_MOM2: return launch_m<K, MODE_MOM2>(R, a, l, st);
     case MODE_MOMX: return launch_m<K, MODE_MOMX>(R, a, l, st);
+    case MODE_CLEN: return launch_m<K, MODE_CLEN>(R, a, l, st);
     }
     return cudaErrorInvalidValue;
 }

@@ -350,3 +350,27 @@ def test_vac_msd_bitwise_reproducible(B, R):
     a = host(B.vac(h, phi, 50, 2, 0.8)); b = host(B.vac(h, phi, 50, 2, 0.8))
     c = host(B.msd(h, phi, 50, 2, 0.8)); d = host(B.msd(h, phi, 50, 2, 0.8))
     assert a.tobytes() == b.tobytes() and c.tobytes() == d.tobytes()
+
+
+@pytest.mark.parametrize("R", [1, 2, 16])
+@pytest.mark.parametrize("dt", [2.1, -0.6, 0.004])
+def test_clenshaw_evolve(B, kgo, R, dt):
+    """U(dt) phi by Clenshaw's backward recurrence (default) against the oracle's literal Alg. 6 and
+    against the library's forward recursion + accumulation; E0 != 0 (global phase), both time
+    directions, and a tiny dt whose series has fewer than 4 terms (falls back to Alg. 6)."""
+    lat = sheet(60, 50, 100, True)                    # 11 900 sites
+    e0 = 0.25
+    s = scale_for(lat) + 0.3
+    olat = to_oracle_lattice(kgo, lat)
+    h = B.from_lattice(lat, lat.x, lat.period_x, e0, s)
+    phi = W.random_phase_vectors(lat.n, R, 13)
+    l0 = h.launch_count
+    out = host(B.evolve(h, dev(phi), dt))
+    n_p, _ = B.bessel_terms(s * abs(dt) / W.HBAR)
+    assert h.launch_count - l0 == n_p - 1             # one sweep per term beyond the first
+    assert relerr(out[:, R - 1], kgo.evolve(olat, e0, s, phi[:, R - 1].copy(), dt)) <= 1e-12
+    h.set_option(B.KG_OPT_CLENSHAW, 0)
+    fwd = host(B.evolve(h, dev(phi), dt))
+    assert relerr(out, fwd) <= 1e-13
+    back = host(B.evolve(h, dev(out), -dt))
+    assert np.max(np.abs(back - phi)) < 1e-12         # U(-dt) U(dt) = 1
