@@ -241,8 +241,10 @@ enum {
     KG_OPT_STAGED_CTAS = 6,  /* CTAs per SM of the staged kernel (0 = auto) */
     KG_OPT_ALTERNATE = 7,    /* 1 (default): alternate the sweep direction step to step (L2 reuse) */
     KG_OPT_DICT = 8,         /* 0: drop the hopping dictionary, stream fp64 hoppings (general path) */
-    KG_OPT_DOUBLING = 9,     /* 1 (default): when phi_L and phi_R are the same array, two moments per
-                                Chebyshev step via 2 T_a T_b = T_{a+b} + T_{|a-b|}; 0: literal Alg. 5 */
+    KG_OPT_DOUBLING = 9,     /* 1 (default): two moments per Chebyshev sweep via 2 T_a T_b = T_{a+b} +
+                                T_{|a-b|} — when phi_L and phi_R are the same array (kg_dos_moments,
+                                kg_msd) and, advancing [phi_L | phi_R] as one batch, in kg_vac;
+                                0: literal Alg. 5 */
     KG_OPT_CLENSHAW = 10     /* 1 (default): U(dt) phi summed by Clenshaw's backward recurrence (no
                                 accumulator stream); 0: forward recursion + accumulation as in Alg. 6 */
 };
