@@ -1,0 +1,48 @@
+"""bench.py keeps the driver's contract: one JSON line with the required keys, on the small config
+(GPU), and the site-update accounting used by both arms (CPU)."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_site_update_accounting():
+    sys.path.insert(0, ROOT)
+    import bench
+    n, R, M, nt, n_p = 1000, 2, 3000, 1, 42
+    lit = bench.site_updates(n, R, M, nt, n_p)
+    dbl = bench.site_updates(n, R, M, nt, n_p, doubling=True)
+    per = n * R
+    assert lit["dos"] == (M - 1) * per                                        # Alg. 5: M - 1 applications
+    assert lit["vac"] == (1 + 2 * (1 + M - 1) + 2 * (n_p - 1)) * per          # Alg. 2, two time points
+    assert lit["msd"] == (2 * (M - 1) + 2 * (n_p - 1)) * per                  # Alg. 3 with the pair recursion
+    assert dbl["dos"] == (M // 2) * per
+    assert dbl["vac"] == (1 + 2 * (1 + 2 * (M // 2)) + 2 * (n_p - 1)) * per   # both chains advanced
+    assert dbl["msd"] == (2 * (M // 2) + 2 * (n_p - 1)) * per
+    assert bench.mom_bytes_per_update(1) == 108.0 and bench.mom_bytes_per_update(8) == 69.5
+    assert bench.mom_bytes_per_update(2, phi_l_stream=False) == 70.0
+
+
+@pytest.mark.gpu
+def test_bench_line_on_small_config():
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--config", "1", "--steps", "2",
+                          "--warmup", "3", "--no-cpu-baseline"], capture_output=True, text=True, cwd=ROOT,
+                         timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [ln for ln in out.stdout.splitlines() if ln.strip()]
+    assert len(lines) == 1                                                    # exactly one JSON line
+    b = json.loads(lines[0])
+    for key in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better",
+                "scaling", "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline"):
+        assert key in b, key
+    assert b["n_gpus"] == 1 and b["steps"] == 2 and b["warmup"] == 3 and b["higher_is_better"] is True
+    assert b["scaling"] == "weak" and b["data"] == "synthetic" and b["vs_baseline"] is None
+    assert "workload" in b["config"] and b["value"] > 0 and b["gpu_launches"] > 0
+    assert set(("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step")) <= set(b["e2e"])
+    assert b["e2e"]["h2d_bytes_per_step"] > 0 and b["e2e"]["d2h_bytes_per_step"] > 0
+    r = b["roofline"]
+    assert r["bound"] == "hbm" and r["unit"] == "GB/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
