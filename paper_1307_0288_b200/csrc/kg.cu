@@ -737,6 +737,33 @@ static int pair_device(kg_hamiltonian *h, const c128 *psi, const c128 *psix, c12
     std::vector<c128> c;
     series_coefficients(h, dt_fs, eps, c);
     const int np = (int)c.size();
+    const StagedPlan cp = staged_plan(h, MODE_PCLEN, R);
+    if (h->clenshaw && cp.ok && np >= 4) {
+        // Clenshaw form of the pair recursion (see evolve_device): b and e chains, np - 1 sweeps,
+        // no accumulator streams; psi_out / psix_out are written by the last sweep.
+        StagedArgs ca = staged_base_args(h, cp);
+        ca.aux = psi; ca.daux = psix;
+        c128 *bb[2] = {(c128 *)ta, (c128 *)tb}, *ee[2] = {(c128 *)da, (c128 *)db};
+        const c128 one = make_double2(1.0, 0.0);
+        for (int m = np - 2, k = 0; m >= 0; --m, ++k) {
+            ca.alpha = m == 0 ? 1.0 : 2.0;
+            ca.next = m == 0 ? psi_out : bb[k & 1];
+            ca.dnext = m == 0 ? psix_out : ee[k & 1];
+            if (k == 0) {
+                ca.cur = psi; ca.prev = psi; ca.dcur = psix; ca.dprev = psix;
+                ca.c1 = c[m]; ca.cpre = c[np - 1]; ca.use_prev = 0;
+            } else if (k == 1) {
+                ca.cur = bb[0]; ca.prev = bb[0]; ca.dcur = ee[0]; ca.dprev = ee[0]; ca.cpre = one; ca.use_prev = 0;
+                ca.c1 = make_double2(c[m].x - c[np - 1].x, c[m].y - c[np - 1].y);
+            } else {
+                ca.cur = bb[(k - 1) & 1]; ca.prev = bb[k & 1]; ca.dcur = ee[(k - 1) & 1]; ca.dprev = ee[k & 1];
+                ca.c1 = c[m]; ca.cpre = one; ca.use_prev = 1;
+            }
+            ca.reverse = h->alternate ? (k & 1) : 0;
+            CUDA_TRY(staged_launch(h, MODE_PCLEN, R, ca, cp, st));
+        }
+        return KG_OK;
+    }
     const StagedPlan sp = staged_plan(h, MODE_PAIR, R);
     StagedArgs sa = staged_base_args(h, sp);
     sa.aux = psi_out; sa.out = psi_out; sa.daux = psix_out; sa.outd = psix_out;

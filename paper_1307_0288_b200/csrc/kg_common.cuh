@@ -15,6 +15,8 @@
 //   MODE_EVO   same recursion + out (+)= c_{m+1} T_{m+1}              (Alg. 6 l.5-6 P:383-385)
 //   MODE_CLEN  (staged kernel only) the same series summed by Clenshaw's backward recurrence
 //              b_m = c_m phi + 2 H~ b_{m+1} - b_{m+2}: no accumulator stream
+//   MODE_PCLEN (staged kernel only) Clenshaw form of the pair recursion (eq 44):
+//              e_m = c_m psix + 2 H~ e_{m+1} + 2 [X,H~] b_{m+1} - e_{m+2} next to b_m
 //   MODE_PAIR  (a, d) pair recursion: a = T_m psi, d = T_m psix + [X,T_m] psi,
 //              d_{m+1} = alpha([X,H~] a_m + H~ d_m) - beta d_{m-1}    (eq 39, Alg. 7 l.7-8)
 //              + both series accumulations                            (eq 44)
@@ -36,7 +38,7 @@
 
 typedef double2 c128;
 
-enum { MODE_MOM = 0, MODE_EVO = 1, MODE_PAIR = 2, MODE_VEL = 3, MODE_MOM2 = 4, MODE_MOMX = 5, MODE_CLEN = 6 };
+enum { MODE_MOM = 0, MODE_EVO = 1, MODE_PAIR = 2, MODE_VEL = 3, MODE_MOM2 = 4, MODE_MOMX = 5, MODE_CLEN = 6, MODE_PCLEN = 7 };
 
 struct StepArgs {
     // matrix (device, library-owned)

@@ -106,13 +106,14 @@ __device__ __forceinline__ void sg_bulk_g2s(uint32_t dst, const void *src, uint3
 
 // Tile size per mode: the pair recursion stages six vector streams, so its tile is half as long
 // to keep >= 2 stages x 3 CTAs per SM in shared memory.
-__host__ __device__ constexpr int sg_tile_e(int mode) { return mode == MODE_PAIR ? 256 : 512; }
-__host__ __device__ constexpr int sg_nvec(int mode) { return mode == MODE_PAIR ? 6 : (mode == MODE_MOM2 || mode == MODE_MOMX) ? 2 : 3; }
+__host__ __device__ constexpr bool sg_is_pair(int mode) { return mode == MODE_PAIR || mode == MODE_PCLEN; }
+__host__ __device__ constexpr int sg_tile_e(int mode) { return sg_is_pair(mode) ? 256 : 512; }
+__host__ __device__ constexpr int sg_nvec(int mode) { return sg_is_pair(mode) ? 6 : (mode == MODE_MOM2 || mode == MODE_MOMX) ? 2 : 3; }
 // bytes of one stage / of the header (host planning and device layout use the same formulas)
 __host__ __device__ constexpr int sg_stage_bytes(int R, int K, int mode, bool ons, bool dict)
 {
     return (sg_nvec(mode) * sg_tile_e(mode) * 16 + (sg_tile_e(mode) / R) * (4 * K + (ons ? 8 : 0) +
-            (mode == MODE_PAIR ? 8 * K : 0) + (dict ? 0 : 8 * K)) + 127) / 128 * 128;
+            (sg_is_pair(mode) ? 8 * K : 0) + (dict ? 0 : 8 * K)) + 127) / 128 * 128;
 }
 // row widths the staged kernels are compiled for (others run kg_step_kernel)
 __host__ __device__ constexpr bool sg_k_supported(int K) { return K == 2 || K == 3 || K == 4 || K == 6; }
@@ -132,7 +133,7 @@ struct SgLayout {
     static constexpr int OFF_IDX = sg_nvec(MODE) * VEC;
     static constexpr int OFF_ONS = OFF_IDX + K * CS * 4;
     static constexpr int OFF_XHOP = OFF_ONS + (ONS ? CS * 8 : 0);
-    static constexpr int OFF_HOP = OFF_XHOP + (MODE == MODE_PAIR ? K * CS * 8 : 0);
+    static constexpr int OFF_HOP = OFF_XHOP + (sg_is_pair(MODE) ? K * CS * 8 : 0);
     static constexpr int STAGE = sg_stage_bytes(R, K, MODE, ONS, DICT);
     static constexpr int OFF_DICT = 2 * SG_MAX_STAGES * 8;
     static constexpr int OFF_RED = OFF_DICT + 16 * 8;
@@ -149,6 +150,9 @@ struct SgLayout {
 // MODE_CLEN  next = c1 phi + cpre (alpha H~ cur) - prev : Clenshaw's backward recurrence for the
 //            series of eq 36, b_m = c_m phi + 2 H~ b_{m+1} - b_{m+2}, U phi = c_0 phi + H~ b_1 - b_2
 //            (aux = phi; three read streams and one write instead of evolve's three and two)
+// MODE_PCLEN the same for the pair of eq 44: b as above and
+//            e_m = c_m psix + 2 H~ e_{m+1} + 2 [X,H~] b_{m+1} - e_{m+2}   (the derivation [X, .] of
+//            Clenshaw's recurrence), psix' = c_0 psix + H~ e_1 + [X,H~] b_1 - e_2; daux = psix
 // MODE_PAIR  the same on the a-chain, and on the d-chain
 //            dnext = 2([X,H~] cur + H~ dcur) - dprev ; outd += c1 dnext  (eq 39, Alg. 7 l.7-8)
 template <int R, int K, int MODE, bool ONS, bool DICT>
@@ -156,7 +160,8 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
 {
     typedef SgLayout<R, K, MODE, ONS, DICT> L;
     constexpr int CS = L::CS, TE = L::TE, EPT = TE / SG_CONSUMERS;
-    constexpr bool PAIR = MODE == MODE_PAIR;
+    constexpr bool PAIR = sg_is_pair(MODE);
+    constexpr bool CLEN = MODE == MODE_CLEN || MODE == MODE_PCLEN;
     extern __shared__ __align__(128) unsigned char sg_smem[];
     uint64_t *bars = reinterpret_cast<uint64_t *>(sg_smem);
     c128 *red = reinterpret_cast<c128 *>(sg_smem + L::OFF_RED);
@@ -310,7 +315,7 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
                 if (le < ne) {
                     const c128 p = prev_s[le];
                     c128 tt;
-                    if (MODE == MODE_CLEN) {
+                    if (CLEN) {
                         const c128 g = cmul(a.cpre, make_double2(a.alpha * acc.x, a.alpha * acc.y));
                         const c128 ca = cmul(a.c1, aux_s[le]);
                         tt = make_double2(ca.x + g.x, ca.y + g.y);
@@ -319,7 +324,7 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
                         tt = make_double2(fma(2.0, acc.x, -p.x), fma(2.0, acc.y, -p.y));
                     }
                     a.next[e0 + le] = tt;
-                    if (MODE == MODE_CLEN) {
+                    if (CLEN) {
                     } else if (MODE == MODE_MOM) {
                         const c128 Lv = aux_s[le];
                         sum.x = fma(Lv.x, tt.x, fma(Lv.y, tt.y, sum.x));      // conj(L) * t
@@ -342,7 +347,14 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
                         const c128 o = aux_s[le], ct = cmul(a.c1, tt);
                         a.out[e0 + le] = make_double2(o.x + ct.x, o.y + ct.y);
                     }
-                    if (PAIR) {
+                    if (MODE == MODE_PCLEN) {
+                        const c128 dp = dprev_s[le];
+                        const c128 g = cmul(a.cpre, make_double2(a.alpha * dacc.x, a.alpha * dacc.y));
+                        const c128 ca = cmul(a.c1, daux_s[le]);
+                        c128 dt = make_double2(ca.x + g.x, ca.y + g.y);
+                        if (a.use_prev) { dt.x -= dp.x; dt.y -= dp.y; }
+                        a.dnext[e0 + le] = dt;
+                    } else if (PAIR) {
                         const c128 dp = dprev_s[le];
                         const c128 dt = make_double2(fma(2.0, dacc.x, -dp.x), fma(2.0, dacc.y, -dp.y));
                         a.dnext[e0 + le] = dt;

@@ -56,6 +56,7 @@ cudaError_t launch_k(int mode, int R, const StagedArgs &a, const StagedLaunch &l
     case MODE_MOM2: return launch_m<K, MODE_MOM2>(R, a, l, st);
     case MODE_MOMX: return launch_m<K, MODE_MOMX>(R, a, l, st);
     case MODE_CLEN: return launch_m<K, MODE_CLEN>(R, a, l, st);
+    case MODE_PCLEN: return launch_m<K, MODE_PCLEN>(R, a, l, st);
     }
     return cudaErrorInvalidValue;
 }

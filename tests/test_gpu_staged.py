@@ -374,3 +374,33 @@ def test_clenshaw_evolve(B, kgo, R, dt):
     assert relerr(out, fwd) <= 1e-13
     back = host(B.evolve(h, dev(out), -dt))
     assert np.max(np.abs(back - phi)) < 1e-12         # U(-dt) U(dt) = 1
+
+
+@pytest.mark.parametrize("R", [1, 8])
+def test_clenshaw_pair(B, kgo, R):
+    """Eq 44 by the Clenshaw form of the (b, e) pair recursion (default) against the oracle's literal
+    Alg. 6 + Alg. 7 over two steps (non-zero psix on the second) and against the forward pair
+    recursion; then MSD moments through it."""
+    lat = sheet(60, 50, 100, True)
+    s = scale_for(lat)
+    olat = to_oracle_lattice(kgo, lat)
+    h = B.from_lattice(lat, lat.x, lat.period_x, 0.0, s)
+    phi = W.random_phase_vectors(lat.n, R, 17)
+    dt = 1.9
+    psi, psix = dev(phi), dev(np.zeros_like(phi))
+    for _ in range(2):
+        B.evolve_x(h, psi, psix, dt)
+    r = R - 1
+    wp, wx = phi[:, r].copy(), np.zeros(lat.n, complex)
+    for _ in range(2):
+        wx = kgo.evolve(olat, 0.0, s, wx, dt) + kgo.comm_evolve(olat, olat.x, olat.period_x, 0.0, s, wp, dt)
+        wp = kgo.evolve(olat, 0.0, s, wp, dt)
+    assert relerr(host(psi)[:, r], wp) <= 1e-12 and relerr(host(psix)[:, r], wx) <= 1e-12
+    msd = host(B.msd(h, dev(phi), 24, 2, dt))
+    h.set_option(B.KG_OPT_CLENSHAW, 0)
+    p2, x2 = dev(phi), dev(np.zeros_like(phi))
+    for _ in range(2):
+        B.evolve_x(h, p2, x2, dt)
+    assert relerr(host(psix), host(x2)) <= 1e-13 and relerr(host(psi), host(p2)) <= 1e-13
+    assert relerr(msd, host(B.msd(h, dev(phi), 24, 2, dt))) <= 1e-12
+    assert relerr(msd[r], kgo.msd(olat, olat.x, olat.period_x, 0.0, s, phi[:, r].copy(), 24, 2, dt)) <= TOL
