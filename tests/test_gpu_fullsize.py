@@ -114,3 +114,35 @@ def test_full_recursion_depth_M3000(B, kgo):
     assert relerr(mom, kgo.moments(olat, 0.0, s, b, a, M)) <= TOL
     vac = host(B.vac(h, dev(a), M, 0, 1.0))[0]
     assert relerr(vac, kgo.vac(olat, olat.x, olat.period_x, 0.0, s, a, M, 0, 1.0)) <= TOL
+
+
+def test_fig2_kpm_and_ftm_dos_agree_at_scale(B):
+    """The paper's own validation (Fig. 2), on the GPU and without the oracle: DOS of a
+    graphene sheet with 1 % vacancies by the KPM (kg_dos_moments -> kg_kpm_reconstruct) and by the
+    FTM (kg_fourier_moments -> kg_ftm_reconstruct, dtau = pi hbar / s as in P:474) from the same
+    four random vectors — two independent kernel chains (recursion + dot vs Clenshaw evolution +
+    inner product).  512 x 256 cells = 524 288 sites before the vacancies.  Compared where the
+    different broadenings drop out: the integrated DOS; plus the vacancy zero-mode peak at E = 0."""
+    full = W.honeycomb(512, 256)
+    lat = W.remove_sites(full, W.vacancy_mask(full.n, W.n_vacancies(0.01, full.n), 7))
+    s = 3 * 2.7 * 1.05
+    h = B.from_lattice(lat, lat.x, lat.period_x, 0.0, s)
+    R = 4
+    phi = dev(W.random_phase_vectors(lat.n, R, 3))
+    en = np.linspace(-8.4, 8.4, 1681)
+    d_en = dev(en)
+    M, Nm = 600, 200
+    dtau = np.pi * W.HBAR / s
+    rho_k = host(B.kpm_reconstruct(B.dos_moments(h, phi, M), 0.0, s, d_en)).mean(axis=0)
+    F = B.fourier_moments(h, phi, phi, Nm, dtau)
+    rho_f = host(B.ftm_reconstruct(F, dtau, d_en)).mean(axis=0)
+    de = en[1] - en[0]
+    n_k, n_f = np.cumsum(rho_k) * de, np.cumsum(rho_f) * de
+    assert abs(n_k[-1] - 1.0) < 2e-3 and abs(n_f[-1] - 1.0) < 2e-3
+    assert np.max(np.abs(n_k - n_f)) < 5e-3
+    Fh = host(F)
+    assert np.max(np.abs(Fh[:, Nm] - 1.0)) < 1e-12                      # F_0 = <phi|phi>
+    assert np.max(np.abs(Fh[:, ::-1] - np.conj(Fh))) < 1e-11            # F_{-n} = conj(F_n)
+    # 1 % vacancies on random sublattices leave zero modes: a DOS peak at E = 0 above its surroundings
+    mid, side = np.abs(en) < 0.05, (np.abs(en) > 0.3) & (np.abs(en) < 0.5)
+    assert rho_k[mid].max() > 2 * rho_k[side].mean() and rho_f[mid].max() > 2 * rho_f[side].mean()
