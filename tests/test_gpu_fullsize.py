@@ -146,3 +146,32 @@ def test_fig2_kpm_and_ftm_dos_agree_at_scale(B):
     # 1 % vacancies on random sublattices leave zero modes: a DOS peak at E = 0 above its surroundings
     mid, side = np.abs(en) < 0.05, (np.abs(en) > 0.3) & (np.abs(en) < 0.5)
     assert rho_k[mid].max() > 2 * rho_k[side].mean() and rho_f[mid].max() > 2 * rho_f[side].mean()
+
+
+def test_einstein_equals_green_kubo_in_the_diffusive_regime(B):
+    """P:532 / P:626: "sigma_E1(E,t) and sigma_GK(E,t) are equivalent" — checked on the GPU without
+    the oracle, through two independent kernel chains: kg_vac (velocity, Clenshaw evolution of the
+    [psi|chi] batch, cross-doubling moment sweeps) against kg_msd (Clenshaw pair recursion of
+    eq 44, doubling moment sweeps), both reconstructed and post-processed on the device.
+    160 000-site sheet with Anderson disorder W = 2|t|, 8 random vectors, dt = 0.1 fs as in the
+    paper's Fig. 5.  d/dt DeltaX^2 / 2 = int_0^t C_vv is exact in the trace, so the two
+    running conductivities agree up to the stochastic error and the O(dt^2) quadrature error."""
+    import torch
+    lat = W.honeycomb(200, 200)
+    lat.onsite = W.anderson(lat.n, 2 * 2.7, 5)
+    s = (3 * 2.7 + 2.7) * 1.05
+    h = B.from_lattice(lat, lat.x, lat.period_x, 0.0, s)
+    R, M, nt, dt = 8, 200, 40, 0.1
+    phi = dev(W.random_phase_vectors(lat.n, R, 9))
+    en = torch.linspace(-3.0, 3.0, 61, dtype=torch.float64).cuda()
+    rho = B.kpm_reconstruct(B.dos_moments(h, phi, M), 0.0, s, en).mean(dim=0).contiguous()
+    fvac = B.kpm_reconstruct(B.vac(h, phi, M, nt, dt), 0.0, s, en).mean(dim=0).contiguous()
+    fmsd = B.kpm_reconstruct(B.msd(h, phi, M, nt, dt), 0.0, s, en).mean(dim=0).contiguous()
+    t = B.transport(rho, fvac, fmsd, dt, 8.0 / (3 * np.sqrt(3) * 0.142 ** 2), 1.0)
+    gk, e1, e2 = host(t["sigma_gk"]), host(t["sigma_e1"]), host(t["sigma_e2"])
+    for k in (10, 20, 39):
+        assert abs(e1[k].mean() / gk[k].mean() - 1.0) < 0.01
+        assert np.linalg.norm(e1[k] - gk[k]) / np.linalg.norm(gk[k]) < 0.05
+    assert np.all(gk[1:] > 0)
+    # sigma_E2 = DeltaX^2 / 2t lags behind sigma_E1 while the VAC is still decaying (P:532)
+    assert 0.5 < e2[39].mean() / e1[39].mean() < 1.5
