@@ -175,3 +175,31 @@ def test_einstein_equals_green_kubo_in_the_diffusive_regime(B):
     assert np.all(gk[1:] > 0)
     # sigma_E2 = DeltaX^2 / 2t lags behind sigma_E1 while the VAC is still decaying
     assert 0.5 < e2[39].mean() / e1[39].mean() < 1.5
+
+
+def test_minimum_conductivity_plateau_of_the_paper(B):
+    """A value the paper prints (Fig. 6; tests/golden/paper_values.txt): for graphene with
+    1 % vacancies the semiclassical conductivity sigma_sc(E) = max_t sigma_E1(E,t) (eq 53) has
+    a plateau at 4e^2/(pi h) = 1.273 e^2/h for |E| < 0.25 eV.  Reproduced end to end on the GPU at
+    the paper's sample size (2048 x 1024 atoms = 1024 x 512 cells, 2.08 M sites after the
+    vacancies), N_m = 3000, 8 random vectors (the paper: 30), kg_msd -> kg_kpm_reconstruct ->
+    kg_transport.  Also the localisation the paper describes: the REC decays after its maximum."""
+    import torch
+    from helpers import golden
+    want, tol = golden("sigma_sc_plateau_e2h")
+    full = W.honeycomb(1024, 512)
+    lat = W.remove_sites(full, W.vacancy_mask(full.n, W.n_vacancies(0.01, full.n), 21))
+    s = 3 * 2.7 * 1.05
+    h = B.from_lattice(lat, lat.x, lat.period_x, 0.0, s)
+    R, M, nt, dt = 8, 3000, 24, 2.0
+    phi = dev(W.random_phase_vectors(lat.n, R, 5))
+    en = torch.linspace(-0.25, 0.25, 21, dtype=torch.float64).cuda()
+    rho = B.kpm_reconstruct(B.dos_moments(h, phi, M), 0.0, s, en).mean(dim=0).contiguous()
+    fmsd = B.kpm_reconstruct(B.msd(h, phi, M, nt, dt), 0.0, s, en).mean(dim=0).contiguous()
+    t = B.transport(rho, None, fmsd, dt, 8.0 / (3 * np.sqrt(3) * 0.142 ** 2), 1.0)
+    e1, e = host(t["sigma_e1"]), host(en)
+    window = np.abs(e) > 0.05                      # E = 0 itself is the vacancy zero-mode peak
+    sigma_sc = e1.max(axis=0)
+    assert abs(sigma_sc[window].mean() - want) <= tol
+    assert np.all(np.abs(sigma_sc[window] - want) < 0.25)
+    assert np.all(e1[-2][window] < 0.8 * sigma_sc[window])          # decaying REC: localisation
