@@ -232,3 +232,38 @@ def test_fig3_length_saturates_at_the_sample_length(B):
     v = np.diff(pbc, axis=0) / dt                                            # constant velocity 2 sqrt(v^2(E))
     assert np.all(np.abs(v[10:] / v[10:].mean(axis=0) - 1.0) < 0.02)
     assert np.max(np.abs(open_[4] - pbc[4]) / pbc[4]) < 0.12                 # early times: same ballistic rise
+
+
+def test_fig4_quantised_conductance_of_the_ribbon(B):
+    """Ballistic regime (sec 5.1, Fig. 4) on config 3's ribbon (30-dimer-line AGNR, 1.2 M
+    sites): the Einstein conductance G = (W/L) sigma_E1 (eqs 50-51) reproduces the conductance
+    quantum staircase — N open channels give N x 2e^2/h — "within a short correlation time", with
+    the slight overestimate towards the band edges that the paper reports.  The channel count is
+    the textbook one for an armchair ribbon of N_a = 30 dimer lines: transverse modes
+    q_p = p pi/(N_a+1), and the pair (p, N_a+1-p) spans |t| |1 - 2|cos q_p|| <= |E| <= |t| (1 + 2|cos q_p|)."""
+    import torch
+    cfg = W.make_config(3)
+    lat = cfg.lattice
+    h = B.from_lattice(lat, cfg.xcoord, cfg.period, 0.0, cfg.scale)
+    t_hop, Na = 2.7, 30
+    c = np.abs(np.cos(np.arange(1, Na // 2 + 1) * np.pi / (Na + 1)))
+    lo, hi = t_hop * np.abs(1 - 2 * c), t_hop * (1 + 2 * c)
+    channels = lambda E: int(np.sum((lo <= abs(E)) & (abs(E) <= hi)))
+    edges = np.sort(lo)
+    mids = 0.5 * (edges[:5] + edges[1:6])                     # centres of the first five plateaus
+    e = np.concatenate([-mids[::-1], [-0.08, 0.0, 0.08], mids])
+    R, M, nt, dt = 4, 2000, 24, 4 * cfg.dt_fs
+    phi = dev(W.random_phase_vectors(lat.n, R, 5))
+    en = torch.from_numpy(e).cuda()
+    rho = B.kpm_reconstruct(B.dos_moments(h, phi, M), 0.0, cfg.scale, en).mean(dim=0).contiguous()
+    fmsd = B.kpm_reconstruct(B.msd(h, phi, M, nt, dt), 0.0, cfg.scale, en).mean(dim=0).contiguous()
+    tr = B.transport(rho, None, fmsd, dt, 2.0 * lat.n / cfg.period, 1.0)
+    g = host(tr["conductance"]) / 2.0                          # in units of 2e^2/h
+    want = np.array([channels(x) for x in e], float)
+    assert list(want[-5:]) == [1, 2, 3, 4, 5] and np.all(want[5:8] == 0)
+    for k in (8, 16, 23):                                      # time-independent after a short time
+        assert np.all(np.abs(g[k][want == 0]) < 0.02)          # the gap of the 3p ribbon
+        ratio = g[k][want > 0] / want[want > 0]
+        assert np.all(ratio > 0.90) and np.all(ratio < 1.12), (k, ratio)     # measured 0.93-1.08 (4 vectors)
+    e2_over_e1 = host(tr["sigma_e2"])[23][want > 0] / host(tr["sigma_e1"])[23][want > 0]
+    assert np.all(np.abs(e2_over_e1 - 0.5) < 0.03)            # sigma_E2 = sigma_E1 / 2 when ballistic (P:519)
