@@ -245,9 +245,12 @@ enum {
                                 T_{|a-b|} — when phi_L and phi_R are the same array (kg_dos_moments,
                                 kg_msd) and, advancing [phi_L | phi_R] as one batch, in kg_vac;
                                 0: literal Alg. 5 */
-    KG_OPT_CLENSHAW = 10     /* 1 (default): U(dt) phi and the pair of eq 44 summed by Clenshaw's backward
+    KG_OPT_CLENSHAW = 10,    /* 1 (default): U(dt) phi and the pair of eq 44 summed by Clenshaw's backward
                                 recurrence (no accumulator streams); 0: forward recursion + accumulation
                                 as in Alg. 6 / Alg. 7 */
+    KG_OPT_PDL = 11          /* consecutive sweeps chained by programmatic dependent launch (the next sweep's
+                                CTAs are scheduled while this one drains): 1 on, 0 off, -1 (default) on for
+                                launch-bound sizes, n * R <= 2^18 */
 };
 int kg_set_option(kg_hamiltonian *h, int option, int64_t value);
 

@@ -28,6 +28,7 @@ KG_OK, KG_EINVAL, KG_ENOMEM, KG_ECUDA, KG_ESPECTRUM, KG_EUNSUPPORTED = range(6)
 KG_OPT_USE_GRAPHS, KG_OPT_BLOCKS_PER_SM, KG_OPT_THREADS = 1, 2, 3
 KG_OPT_STAGED, KG_OPT_STAGES, KG_OPT_STAGED_CTAS, KG_OPT_ALTERNATE, KG_OPT_DICT, KG_OPT_DOUBLING = 4, 5, 6, 7, 8, 9
 KG_OPT_CLENSHAW = 10
+KG_OPT_PDL = 11
 
 _vp, _i64, _i32, _dbl, _int = C.c_void_p, C.c_int64, C.c_int32, C.c_double, C.c_int
 _lib.kg_last_error.restype = C.c_char_p

@@ -66,7 +66,7 @@ struct kg_hamiltonian {
     double *hop, *xhop, *onsite;
     double dict[16];          // hopping dictionary, dict[0] = 0
     int ndict;                // entries in use (0: hoppings do not fit a dictionary)
-    int staged, stages, staged_ctas, alternate, doubling, clenshaw;   // options of the staged kernel
+    int staged, stages, staged_ctas, alternate, doubling, clenshaw, pdl;   // options of the staged kernel
     void *ws[WS_COUNT];
     size_t ws_bytes[WS_COUNT];
     size_t matrix_bytes;
@@ -191,6 +191,9 @@ static cudaError_t staged_launch(kg_hamiltonian *h, int mode, int R, const Stage
     h->launches++;
     StagedLaunch l;
     l.grid = p.grid; l.smem = p.smem; l.device = h->device; l.has_onsite = h->has_onsite; l.dict = h->ndict > 0;
+    // programmatic dependent launch pays where launch latency dominates (config 1: 4.1 -> 2.8 us per
+    // sweep); on multi-megabyte sweeps it was measured slower (config 4 MOM2 43 -> 52 us)
+    l.pdl = h->pdl > 0 || (h->pdl < 0 && h->n * (int64_t)R <= ((int64_t)1 << 18));
     switch (h->kmax) {
     case 2: return kg_staged_launch_k2(mode, R, a, l, st);
     case 3: return kg_staged_launch_k3(mode, R, a, l, st);
@@ -326,7 +329,7 @@ static int create_from_device_list(kg_hamiltonian **out, int64_t n, int kmax, co
     h->n = n; h->ns = (n + SG_TILE_E - 1) / SG_TILE_E * SG_TILE_E; h->kmax = kmax;
     h->s = s; h->e0 = e0; h->period = period;
     h->nl = h->nlp = nullptr; h->hop = h->xhop = h->onsite = nullptr;
-    h->ndict = 0; h->staged = 1; h->stages = 0; h->staged_ctas = 0; h->alternate = 1; h->doubling = 1; h->clenshaw = 1;
+    h->ndict = 0; h->staged = 1; h->stages = 0; h->staged_ctas = 0; h->alternate = 1; h->doubling = 1; h->clenshaw = 1; h->pdl = -1;
     memset(h->dict, 0, sizeof(h->dict));
     memset(h->ws, 0, sizeof(h->ws));
     memset(h->ws_bytes, 0, sizeof(h->ws_bytes));
@@ -546,6 +549,7 @@ extern "C" int kg_set_option(kg_hamiltonian *h, int option, int64_t value)
     case KG_OPT_ALTERNATE: h->alternate = value != 0; break;
     case KG_OPT_DOUBLING: h->doubling = value != 0; break;
     case KG_OPT_CLENSHAW: h->clenshaw = value != 0; break;
+    case KG_OPT_PDL: h->pdl = value < 0 ? -1 : (value != 0); break;
     case KG_OPT_DICT:
         if (value != 0) return fail(KG_EINVAL, "the dictionary can only be switched off");
         h->ndict = 0; break;

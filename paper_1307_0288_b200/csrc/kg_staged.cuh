@@ -170,6 +170,10 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
     const int tid = threadIdx.x;
     const int nst = a.nstages;
     const uint32_t full0 = sg_smem_u32(bars), empty0 = sg_smem_u32(bars + SG_MAX_STAGES);
+    // Programmatic dependent launch: let the next sweep's CTAs be scheduled as ours drain, and do
+    // our own set-up (barrier init) while the previous sweep is still finishing; nothing that the
+    // previous kernel wrote is touched before griddepcontrol.wait.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if (tid == 0) {
         for (int s = 0; s < nst; ++s) {
             sg_mbar_init(full0 + 8 * s, 1);
@@ -178,6 +182,7 @@ __global__ void __launch_bounds__(SG_THREADS) kg_staged_kernel(const StagedArgs 
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
+    asm volatile("griddepcontrol.wait;" ::: "memory");
 
     const int64_t total = a.n * R;
     const int my_tiles = ((int)blockIdx.x < a.ntiles) ? (a.ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;

@@ -20,8 +20,21 @@ cudaError_t launch_t(const StagedArgs &a, const StagedLaunch &l, cudaStream_t st
         if (e != cudaSuccess) return e;
         configured[dev] = l.smem;
     }
-    kg_staged_kernel<R, K, MODE, ONS, DICT><<<l.grid, SG_THREADS, l.smem, st>>>(a);
-    return cudaGetLastError();
+    if (!l.pdl) {
+        kg_staged_kernel<R, K, MODE, ONS, DICT><<<l.grid, SG_THREADS, l.smem, st>>>(a);
+        return cudaGetLastError();
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)l.grid);
+    cfg.blockDim = dim3(SG_THREADS);
+    cfg.dynamicSmemBytes = l.smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kg_staged_kernel<R, K, MODE, ONS, DICT>, a);
 }
 
 template <int R, int K, int MODE>

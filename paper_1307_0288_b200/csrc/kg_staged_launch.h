@@ -11,6 +11,7 @@ struct StagedLaunch {
     int device;
     bool has_onsite;      // ONS template flag
     bool dict;            // DICT template flag
+    bool pdl;             // launch with programmatic stream serialization
 };
 
 // mode: MODE_MOM / MODE_EVO / MODE_PAIR / MODE_MOM2 / MODE_MOMX; R: columns of the batch.
