@@ -412,9 +412,14 @@ int kgo_dos_moments(int64_t n, int kmax, const int32_t *nn, const int32_t *nl,
 /* chi_{k+1} = U(-dt) chi_k  (time grid t_k = k dt, reading g8).               */
 /* mu is [n_steps+1][M].                                                       */
 /* ------------------------------------------------------------------------- */
-int kgo_vac(int64_t n, int kmax, const int32_t *nn, const int32_t *nl, const double *hop,
-            const double *onsite, const double *x, double period, double e0, double s,
-            const kgo_c *phi, int M, int n_steps, double dt_fs, double eps, kgo_c *mu)
+/* Row k holds Mk[k] moments (Mk[k] = 0: no moments at t_k, the states are only advanced);  */
+/* row stride ld.  Chebyshev moments do not depend on how many of them are asked for, so a   */
+/* shorter row is a prefix of the longer one: tests/golden/make_goldens.py uses this to      */
+/* tabulate all time steps of the large configs with a short prefix and full rows at the ends. */
+int kgo_vac_sched(int64_t n, int kmax, const int32_t *nn, const int32_t *nl, const double *hop,
+                  const double *onsite, const double *x, double period, double e0, double s,
+                  const kgo_c *phi, int n_steps, const int *Mk, int ld, double dt_fs, double eps,
+                  kgo_c *mu)
 {
     const size_t bytes = (size_t)n * sizeof(kgo_c);
     kgo_c *psi = (kgo_c *)malloc(bytes), *chi = (kgo_c *)malloc(bytes);
@@ -424,9 +429,11 @@ int kgo_vac(int64_t n, int kmax, const int32_t *nn, const int32_t *nl, const dou
     memcpy(psi, phi, bytes);
     kgo_apply_v(n, kmax, nn, nl, hop, x, period, phi, chi);
     for (int k = 0; k <= n_steps; ++k) {
-        kgo_apply_v(n, kmax, nn, nl, hop, x, period, psi, phiL);
-        rc = kgo_moments(n, kmax, nn, nl, hop, onsite, e0, s, phiL, chi, M, mu + (size_t)k * M);
-        if (rc) goto done;
+        if (Mk[k] > 0) {
+            kgo_apply_v(n, kmax, nn, nl, hop, x, period, psi, phiL);
+            rc = kgo_moments(n, kmax, nn, nl, hop, onsite, e0, s, phiL, chi, Mk[k], mu + (size_t)k * ld);
+            if (rc) goto done;
+        }
         if (k == n_steps) break;
         rc = kgo_evolve(n, kmax, nn, nl, hop, onsite, e0, s, psi, -fabs(dt_fs), eps, nxt);
         if (rc) goto done;
@@ -440,15 +447,30 @@ done:
     return rc;
 }
 
+int kgo_vac(int64_t n, int kmax, const int32_t *nn, const int32_t *nl, const double *hop,
+            const double *onsite, const double *x, double period, double e0, double s,
+            const kgo_c *phi, int M, int n_steps, double dt_fs, double eps, kgo_c *mu)
+{
+    int *Mk = (int *)malloc((size_t)(n_steps + 1) * sizeof(int));
+    if (!Mk) return 1;
+    for (int k = 0; k <= n_steps; ++k) Mk[k] = M;
+    const int rc = kgo_vac_sched(n, kmax, nn, nl, hop, onsite, x, period, e0, s, phi, n_steps, Mk, M,
+                                 dt_fs, eps, mu);
+    free(Mk);
+    return rc;
+}
+
 /* ------------------------------------------------------------------------- */
 /* O8. MSD moments (Alg. 3; eqs 34, 44).                             */
 /* psi_0 = phi, psix_0 = 0.  For k = 0..n_steps: mu[k][:] = moments with       */
 /* phi_L = phi_R = psix_k; then                                                */
 /* psix_{k+1} = U(dt) psix_k + [X,U(dt)] psi_k  (eq 44),  psi_{k+1} = U(dt)psi_k. */
 /* ------------------------------------------------------------------------- */
-int kgo_msd(int64_t n, int kmax, const int32_t *nn, const int32_t *nl, const double *hop,
-            const double *onsite, const double *x, double period, double e0, double s,
-            const kgo_c *phi, int M, int n_steps, double dt_fs, double eps, kgo_c *mu)
+/* Per-row moment counts Mk[k] and row stride ld as in kgo_vac_sched. */
+int kgo_msd_sched(int64_t n, int kmax, const int32_t *nn, const int32_t *nl, const double *hop,
+                  const double *onsite, const double *x, double period, double e0, double s,
+                  const kgo_c *phi, int n_steps, const int *Mk, int ld, double dt_fs, double eps,
+                  kgo_c *mu)
 {
     const size_t bytes = (size_t)n * sizeof(kgo_c);
     kgo_c *psi = (kgo_c *)malloc(bytes), *psix = (kgo_c *)malloc(bytes);
@@ -458,8 +480,10 @@ int kgo_msd(int64_t n, int kmax, const int32_t *nn, const int32_t *nl, const dou
     memcpy(psi, phi, bytes);
     memset(psix, 0, bytes);
     for (int k = 0; k <= n_steps; ++k) {
-        rc = kgo_moments(n, kmax, nn, nl, hop, onsite, e0, s, psix, psix, M, mu + (size_t)k * M);
-        if (rc) goto done;
+        if (Mk[k] > 0) {
+            rc = kgo_moments(n, kmax, nn, nl, hop, onsite, e0, s, psix, psix, Mk[k], mu + (size_t)k * ld);
+            if (rc) goto done;
+        }
         if (k == n_steps) break;
         rc = kgo_evolve(n, kmax, nn, nl, hop, onsite, e0, s, psix, fabs(dt_fs), eps, a);
         if (rc) goto done;
@@ -472,6 +496,19 @@ int kgo_msd(int64_t n, int kmax, const int32_t *nn, const int32_t *nl, const dou
     }
 done:
     free(psi); free(psix); free(a); free(b);
+    return rc;
+}
+
+int kgo_msd(int64_t n, int kmax, const int32_t *nn, const int32_t *nl, const double *hop,
+            const double *onsite, const double *x, double period, double e0, double s,
+            const kgo_c *phi, int M, int n_steps, double dt_fs, double eps, kgo_c *mu)
+{
+    int *Mk = (int *)malloc((size_t)(n_steps + 1) * sizeof(int));
+    if (!Mk) return 1;
+    for (int k = 0; k <= n_steps; ++k) Mk[k] = M;
+    const int rc = kgo_msd_sched(n, kmax, nn, nl, hop, onsite, x, period, e0, s, phi, n_steps, Mk, M,
+                                 dt_fs, eps, mu);
+    free(Mk);
     return rc;
 }
 

@@ -218,6 +218,28 @@ def msd(lat, xcoord, period, e0, s, phi, M, n_steps, dt_fs, eps=1e-15):
     return mu
 
 
+def _sched(fn, lat, xcoord, period, e0, s, phi, Mk, dt_fs, eps):
+    phi = _c128(phi); xc = _f64(xcoord)
+    Mk = np.ascontiguousarray(Mk, dtype=np.int32)
+    n_steps, ld = Mk.shape[0] - 1, int(Mk.max())
+    mu = np.zeros((n_steps + 1, ld), np.complex128)
+    rc = fn(*_lat_args(lat), _p(lat.onsite), _p(xc), C.c_double(period), C.c_double(e0),
+            C.c_double(s), _p(phi), C.c_int(n_steps), _p(Mk), C.c_int(ld), C.c_double(dt_fs),
+            C.c_double(eps), _p(mu))
+    assert rc == 0
+    return mu
+
+
+def vac_sched(lat, xcoord, period, e0, s, phi, Mk, dt_fs, eps=1e-15):
+    """kgo_vac with Mk[k] moments at time step k (0 = none); returns [len(Mk)][max Mk], unused
+    entries 0."""
+    return _sched(lib().kgo_vac_sched, lat, xcoord, period, e0, s, phi, Mk, dt_fs, eps)
+
+
+def msd_sched(lat, xcoord, period, e0, s, phi, Mk, dt_fs, eps=1e-15):
+    return _sched(lib().kgo_msd_sched, lat, xcoord, period, e0, s, phi, Mk, dt_fs, eps)
+
+
 def jackson(M):
     g = np.empty(M)
     lib().kgo_jackson(C.c_int(M), _p(g))
