@@ -50,6 +50,14 @@ def mom_bytes_per_update(R: int, kmax: int = 3, phi_l_stream: bool = True) -> fl
     return 48.0 + (16.0 if phi_l_stream else 0.0) + (kmax * 12.0 + 8.0) / R
 
 
+def must_move_bytes_per_update(R: int, kmax: int = 3, onsite: bool = True, dictionary: bool = True) -> float:
+    """What the LAUNCHED doubling sweep has to move through HBM with no cache reuse between launches:
+    T_m and T_{m-1} read, T_{m+1} written (48 B per element) + the matrix row shared by the R columns:
+    4 B packed index per neighbour (the fp64 hopping rides in the index word when the hopping
+    dictionary applies, else + 8 B) + 8 B on-site energy when the model has a diagonal."""
+    return 48.0 + (kmax * (4.0 if dictionary else 12.0) + (8.0 if onsite else 0.0)) / R
+
+
 def site_updates(n: int, R: int, M: int, nt: int, n_p: int, doubling: bool = False) -> dict:
     """H~-applications one step really performs.  The oracle runs the literal
     Alg. 5 (M-1 applications per moment set); the CUDA path gets two moments per sweep from the
@@ -58,7 +66,8 @@ def site_updates(n: int, R: int, M: int, nt: int, n_p: int, doubling: bool = Fal
     per_set = M // 2 if doubling else M - 1
     dos = per_set
     vac = 1 + (nt + 1) * (1 + (2 * (M // 2) if doubling else M - 1)) + nt * 2 * (n_p - 1)
-    msd = (nt + 1) * per_set + nt * 2 * (n_p - 1)
+    # MSD row k = 0 is exactly 0 (psix_0 = 0) and is written, not computed: nt moment sets
+    msd = nt * per_set + nt * 2 * (n_p - 1)
     per_vec = {"dos": dos, "vac": vac, "msd": msd}
     return {k: v * n * R for k, v in per_vec.items()}
 
@@ -132,24 +141,31 @@ class ClockSampler:
 # --------------------------------------------------------------------------------------
 # oracle legs (cpu_baseline, --impl reference): the only places bench.py executes oracle/
 # --------------------------------------------------------------------------------------
-ORACLE_SAMPLE = {"dos_M": 33, "corr_M": 2, "nt": 1}
+# SURVEY 8(d) "CPU baseline": K consecutive steps of recursion + dot (Alg. 5: kgo_apply_h, the
+# axpy of l.6 and the long-double inner product of l.7) on the config's own lattice, one vector,
+# single-threaded oracle as it stands.  The same sample in both legs; site-updates = the H~
+# applications the oracle really executes (kgo_moments with M moments calls kgo_apply_h M - 1 times).
+ORACLE_SAMPLE_M = 101
 
 
-def oracle_step(cfg, olat, phi, sample):
-    """One bounded sample of the step on the host, single-threaded oracle."""
+def oracle_step(cfg, olat, phi, m_sample=ORACLE_SAMPLE_M):
     from oracle import kgo
-    kgo.dos_moments(olat, cfg.e0, cfg.scale, phi, sample["dos_M"])
-    kgo.vac(olat, cfg.xcoord, cfg.period, cfg.e0, cfg.scale, phi, sample["corr_M"], sample["nt"], cfg.dt_fs)
-    kgo.msd(olat, cfg.xcoord, cfg.period, cfg.e0, cfg.scale, phi, sample["corr_M"], sample["nt"], cfg.dt_fs)
+    kgo.moments(olat, cfg.e0, cfg.scale, phi, phi, m_sample)
 
 
-def oracle_units(cfg, sample):
-    from oracle import kgo
-    n_p = kgo.bessel_np(cfg.scale * cfg.dt_fs / 0.6582119569)
-    n = cfg.lattice.n
-    d = site_updates(n, 1, sample["dos_M"], 0, n_p)["dos"]
-    c = site_updates(n, 1, sample["corr_M"], sample["nt"], n_p)
-    return d + c["vac"] + c["msd"]
+def oracle_units(cfg, m_sample=ORACLE_SAMPLE_M):
+    return (m_sample - 1) * cfg.lattice.n
+
+
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.lower().startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
 
 
 def oracle_inputs(cfg):
@@ -163,10 +179,17 @@ def oracle_inputs(cfg):
     return olat, phi
 
 
-def sample_text(cfg, sample):
-    return (f"{cfg.name} lattice ({cfg.lattice.n} sites), 1 vector: dos M={sample['dos_M']}; vac and msd "
-            f"M={sample['corr_M']}, {sample['nt']} time step (dt = 4 hbar/|t|, N_p = 42); "
-            "site-updates counted as in the GPU arm")
+def sample_text(cfg, m_sample=ORACLE_SAMPLE_M):
+    return (f"{m_sample - 1} consecutive steps of recursion + dot (kgo_moments, literal Alg. 5: kgo_apply_h + axpy + "
+            f"long-double inner product per step) on the {cfg.name} lattice ({cfg.lattice.n} sites), 1 vector, "
+            f"1 thread of '{cpu_model()}' ({os.cpu_count()} logical cores on the host); site-updates = H~ applications "
+            "the oracle executes")
+
+
+def cpu_baseline_block(value, seconds, cfg):
+    return {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": seconds,
+            "cpu_model": cpu_model(), "host_cores_available": os.cpu_count(),
+            "build": "gcc -O2 -ffp-contract=off, no OpenMP (oracle/kgo.py)", "sample": sample_text(cfg)}
 
 
 def run_reference(args, cfg):
@@ -174,20 +197,19 @@ def run_reference(args, cfg):
     if rank != 0:
         return
     olat, phi = oracle_inputs(cfg)
-    units = oracle_units(cfg, ORACLE_SAMPLE)
+    units = oracle_units(cfg)
     for _ in range(args.warmup):
-        oracle_step(cfg, olat, phi, ORACLE_SAMPLE)
+        oracle_step(cfg, olat, phi)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        oracle_step(cfg, olat, phi, ORACLE_SAMPLE)
+        oracle_step(cfg, olat, phi)
     dt = time.perf_counter() - t0
     val = units * args.steps / dt / 1e9
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "c128 (fp64 complex)",
             "data": "synthetic", "config": workload_config(cfg, args, 1),
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle",
-                             "sample": sample_text(cfg, ORACLE_SAMPLE)},
+            "cpu_baseline": cpu_baseline_block(val, dt / args.steps, cfg),
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -297,14 +319,24 @@ def run_b200(args, cfg):
     torch.cuda.synchronize()
     kern_us = e0.elapsed_time(e1) * 1e3 / (reps * (M // 2))
     peak, peak_src = peaks()
-    bytes_launch = mom_bytes_per_update(2 * R, lat.kmax, phi_l_stream=False) * n * 2 * R
+    # numerator: the bytes this variant must move (hopping dictionary: no fp64 hopping stream) — never
+    # more than SURVEY 8(d)'s general-ELL figure, which is reported beside it
+    bytes_launch = must_move_bytes_per_update(2 * R, lat.kmax, lat.onsite is not None) * n * 2 * R
+    bytes_8d = mom_bytes_per_update(2 * R, lat.kmax, phi_l_stream=False) * n * 2 * R
     achieved = bytes_launch / (kern_us * 1e-6) / 1e9
     traffic = ncu_traffic(f"{cfg.name}_momx_R{2 * R}")
     roofline = {"bound": "hbm", "kernel": f"kg_staged_kernel<R={2 * R}, MODE_MOMX> (fused T_m+1 = 2H~T_m - T_m-1 on [phi_L | phi_R] "
                                          "+ <T_m L|T_m+1 R>, <T_m+1 L|T_m+1 R>; TMA-staged streams, hopping dictionary, alternating sweep)",
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0,
-                "algorithmic_bytes_per_launch": bytes_launch, "us_per_launch": kern_us,
+                "bytes_per_launch": bytes_launch,
+                "bytes_definition": "must-move bytes of the launched variant: (48 + (4 K + 8)/R') B per site-update "
+                                    "(T_m, T_m-1 read, T_m+1 written, packed index + on-site row shared by the R' = 2R columns)",
+                "survey_8d_general_ell": {"bytes_per_launch": bytes_8d, "achieved": bytes_8d / (kern_us * 1e-6) / 1e9,
+                                          "frac": bytes_8d / (kern_us * 1e-6) / 1e9 / peak,
+                                          "note": "SURVEY 8(d) doubling row 48 + (12 K + 8)/R' with fp64 hoppings streamed; the "
+                                                  "kernel does not move those 8 K bytes, so this fraction can exceed 1"},
+                "us_per_launch": kern_us,
                 "gsu_per_s": n * 2 * R / (kern_us * 1e-6) / 1e9, "traffic": traffic}
 
     if rank != 0:
@@ -328,13 +360,11 @@ def run_b200(args, cfg):
             "roofline": roofline}
     if world == 1 and not args.no_cpu_baseline:
         olat, phi1 = oracle_inputs(cfg)
-        sample = {"dos_M": 65, "corr_M": 4, "nt": 1}
+        oracle_step(cfg, olat, phi1, 3)                      # touch the pages once
         t0 = time.perf_counter()
-        oracle_step(cfg, olat, phi1, sample)
+        oracle_step(cfg, olat, phi1)
         dt = time.perf_counter() - t0
-        line["cpu_baseline"] = {"value": oracle_units(cfg, sample) / dt / 1e9, "unit": UNIT, "cores": 1,
-                                "kind": "oracle", "seconds": dt, "host_cores_available": os.cpu_count(),
-                                "sample": sample_text(cfg, sample)}
+        line["cpu_baseline"] = cpu_baseline_block(oracle_units(cfg) / dt / 1e9, dt, cfg)
     print(json.dumps(line), flush=True)
     ctx.finalize()
 

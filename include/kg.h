@@ -248,11 +248,24 @@ enum {
     KG_OPT_CLENSHAW = 10,    /* 1 (default): U(dt) phi and the pair of eq 44 summed by Clenshaw's backward
                                 recurrence (no accumulator streams); 0: forward recursion + accumulation
                                 as in Alg. 6 / Alg. 7 */
+    KG_OPT_REORDER = 12,     /* process-wide, read at create (kg_set_default_option): re-number the sites
+                                internally so that consecutive sites form compact patches of the lattice
+                                (recursive breadth-first bisection of the neighbour list; moments do not
+                                depend on the site order, vectors are permuted at the boundary of every call):
+                                1 always, 0 never, -1 (default) when n >= 65536 */
+    KG_OPT_TWO_STEP = 13,    /* doubling moment loops on <= 2 contiguous columns run two Chebyshev steps per
+                                pass with the tile + two halo rings in shared memory (temporal blocking):
+                                1 whenever the plan fits, 0 never, -1 (default) when the sites are re-ordered
+                                and there are at least four 1024-element tiles per SM */
     KG_OPT_PDL = 11          /* consecutive sweeps chained by programmatic dependent launch (the next sweep's
                                 CTAs are scheduled while this one drains): 1 on, 0 off, -1 (default) on for
                                 launch-bound sizes, n * R <= 2^18 */
 };
 int kg_set_option(kg_hamiltonian *h, int option, int64_t value);
+
+/* Options that act at create time (KG_OPT_REORDER): process-wide default for handles created
+ * afterwards.  Not thread-safe against concurrent kg_create_hamiltonian calls. */
+int kg_set_default_option(int option, int64_t value);
 
 /* Number of kernel launches (graph nodes included) the handle has enqueued since creation. */
 int64_t kg_launch_count(const kg_hamiltonian *h);

@@ -29,6 +29,8 @@ KG_OPT_USE_GRAPHS, KG_OPT_BLOCKS_PER_SM, KG_OPT_THREADS = 1, 2, 3
 KG_OPT_STAGED, KG_OPT_STAGES, KG_OPT_STAGED_CTAS, KG_OPT_ALTERNATE, KG_OPT_DICT, KG_OPT_DOUBLING = 4, 5, 6, 7, 8, 9
 KG_OPT_CLENSHAW = 10
 KG_OPT_PDL = 11
+KG_OPT_REORDER = 12
+KG_OPT_TWO_STEP = 13
 
 _vp, _i64, _i32, _dbl, _int = C.c_void_p, C.c_int64, C.c_int32, C.c_double, C.c_int
 _lib.kg_last_error.restype = C.c_char_p
@@ -51,6 +53,7 @@ _lib.kg_vac.argtypes = [_vp, _vp, _int, _int, _int, _dbl, _dbl, _vp, _vp]
 _lib.kg_msd.argtypes = [_vp, _vp, _int, _int, _int, _dbl, _dbl, _vp, _vp]
 _lib.kg_bessel_terms.argtypes = [_dbl, _dbl, C.POINTER(_int), _vp, _int]
 _lib.kg_set_option.argtypes = [_vp, _int, _i64]
+_lib.kg_set_default_option.argtypes = [_int, _i64]
 _lib.kg_transport.argtypes = [_int, _int, _dbl, _dbl, _dbl] + [_vp] * 9
 _lib.kg_fourier_moments.argtypes = [_vp, _vp, _vp, _int, _int, _dbl, _dbl, _vp, _vp]
 _lib.kg_ftm_reconstruct.argtypes = [_vp, _i64, _int, _int, _dbl, _vp, _int, _vp, _vp]
@@ -128,6 +131,11 @@ class Hamiltonian:
 
     def set_option(self, option, value):
         _check(_lib.kg_set_option(self._h, option, value))
+
+
+def set_default_option(option, value):
+    """kg_set_default_option: create-time options (KG_OPT_REORDER) for handles created afterwards."""
+    _check(_lib.kg_set_default_option(option, value))
 
 
 def create_hamiltonian(n, kmax, nn, nl, hop_eV, onsite_eV, x_nm, period_x_nm, e0_eV, scale_eV,

@@ -5,6 +5,9 @@
 #include "kg_kernels.cuh"
 #include "kg_staged.cuh"
 #include "kg_staged_launch.h"
+#include "kg_partition.h"
+#include "kg_tb2.cuh"
+#include "kg_tb2_launch.h"
 
 #include <algorithm>
 #include <cmath>
@@ -37,6 +40,19 @@ static int fail(int code, const char *fmt, ...)
 
 extern "C" const char *kg_last_error(void) { return g_err; }
 
+// options read by kg_create_hamiltonian[_csr] (set before create; process-wide)
+static int g_reorder = -1;                    // KG_OPT_REORDER: -1 auto, 0 off, 1 always
+#define KG_REORDER_MIN_SITES ((int64_t)1 << 16)
+#define KG_REORDER_LEAF 64
+
+extern "C" int kg_set_default_option(int option, int64_t value)
+{
+    switch (option) {
+    case KG_OPT_REORDER: g_reorder = value < 0 ? -1 : (value != 0); return KG_OK;
+    }
+    return fail(KG_EINVAL, "kg_set_default_option: option %d has no process-wide default", option);
+}
+
 // --------------------------------------------------------------------------------------
 // handle
 // --------------------------------------------------------------------------------------
@@ -45,7 +61,9 @@ enum {
     WS_S0, WS_S1, WS_X0, WS_X1,            // persistent time-stepping states (D6)
     WS_PHIL,                               // V psi_k (VAC left vector)
     WS_PART,                               // per-block moment partials [M][B][R]
-    WS_IN0, WS_IN1, WS_OUT0, WS_OUT1,      // staging for host-pointer arguments
+    WS_IN0, WS_IN1, WS_OUT0, WS_OUT1,      // internal-order copies of caller vectors (host pointers and / or re-ordered sites)
+    WS_RAW0, WS_RAW1,                      // caller-order staging between a host pointer and the permutation kernel
+    WS_TC, WS_TD,                          // third / fourth Chebyshev vector of the two-step kernel
     WS_MU,                                 // device moments when the caller's mu is host memory
     WS_COUNT
 };
@@ -56,6 +74,17 @@ struct GraphEntry {
     cudaGraphExec_t exec;
 };
 
+// per-tile plan of the two-step kernel (kg_tb2.cuh), one per column count C = 1, 2
+struct Tb2Plan {
+    bool built, ok;
+    int cap1, cap2, ntiles;
+    int2 *tinfo;
+    uint16_t *rows;
+    int32_t *hid;
+    double *hons;
+    size_t bytes;
+};
+
 struct kg_hamiltonian {
     int64_t n, ns;
     int kmax;
@@ -63,10 +92,13 @@ struct kg_hamiltonian {
     bool has_onsite;
     int32_t *nl;
     int32_t *nlp;             // (dictionary id << 28) | NL_ik, for the staged kernel (DICT)
+    int32_t *perm, *iperm;    // site re-ordering (kg_partition.h): internal i = caller perm[i]; NULL: caller order
     double *hop, *xhop, *onsite;
     double dict[16];          // hopping dictionary, dict[0] = 0
     int ndict;                // entries in use (0: hoppings do not fit a dictionary)
     int staged, stages, staged_ctas, alternate, doubling, clenshaw, pdl;   // options of the staged kernel
+    int tb2;                  // KG_OPT_TWO_STEP: -1 auto, 0 off, 1 whenever a plan exists
+    Tb2Plan tbp[2];
     void *ws[WS_COUNT];
     size_t ws_bytes[WS_COUNT];
     size_t matrix_bytes;
@@ -105,16 +137,59 @@ static bool is_device_ptr(const void *p)
     return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
 }
 
-// device view of an input array: the pointer itself, or a staged copy of host memory
-static int stage_in(kg_hamiltonian *h, int slot, const void *p, size_t bytes, cudaStream_t st,
-                    const void **dev)
+static int grid_for(const kg_hamiltonian *h, int64_t elems);
+
+// Internal-order device view of a caller vector [n][R] (host or device pointer, caller's site order):
+// the pointer itself when it is a device pointer and the sites are not re-ordered; else a copy in
+// workspace slot `slot` (host -> device copy and / or the permutation kernel).
+static int vec_in(kg_hamiltonian *h, int slot, const void *p, int R, cudaStream_t st, const void **dev)
 {
-    if (is_device_ptr(p)) { *dev = p; return KG_OK; }
+    const size_t bytes = (size_t)h->n * R * 16;
+    const bool on_dev = is_device_ptr(p);
+    if (on_dev && !h->perm) { *dev = p; return KG_OK; }
     void *d;
     int rc = ws_get(h, slot, bytes, &d);
     if (rc) return rc;
-    CUDA_TRY(cudaMemcpyAsync(d, p, bytes, cudaMemcpyHostToDevice, st));
+    const void *src = p;
+    if (!on_dev) {
+        void *raw = d;
+        if (h->perm && (rc = ws_get(h, WS_RAW0 + (slot == WS_IN1 ? 1 : 0), bytes, &raw))) return rc;
+        CUDA_TRY(cudaMemcpyAsync(raw, p, bytes, cudaMemcpyHostToDevice, st));
+        src = raw;
+    }
+    if (h->perm) {
+        kg_permute_rows<<<grid_for(h, h->n * R), 256, 0, st>>>((const c128 *)src, (c128 *)d, h->perm, h->n, R);
+        h->launches++;
+        CUDA_TRY(cudaGetLastError());
+    }
     *dev = d;
+    return KG_OK;
+}
+
+// Output vector [n][R]: `dev` is the internal-order device buffer the kernels write; vec_out_finish
+// brings it to the caller's array (inverse permutation and / or device -> host copy).
+struct VecOut { void *user; void *dev; int R; int slot; bool host; };
+static int vec_out(kg_hamiltonian *h, int slot, void *p, int R, VecOut *o)
+{
+    o->user = p; o->R = R; o->slot = slot; o->host = !is_device_ptr(p);
+    if (!o->host && !h->perm) { o->dev = p; return KG_OK; }
+    return ws_get(h, slot, (size_t)h->n * R * 16, &o->dev);
+}
+static int vec_out_finish(kg_hamiltonian *h, const VecOut &o, cudaStream_t st)
+{
+    const size_t bytes = (size_t)h->n * o.R * 16;
+    if (!o.host && !h->perm) return KG_OK;
+    const void *src = o.dev;
+    if (h->perm) {
+        void *dst = o.user;
+        int rc;
+        if (o.host && (rc = ws_get(h, WS_RAW0 + (o.slot == WS_OUT1 ? 1 : 0), bytes, &dst))) return rc;
+        kg_permute_rows<<<grid_for(h, h->n * o.R), 256, 0, st>>>((const c128 *)o.dev, (c128 *)dst, h->iperm, h->n, o.R);
+        h->launches++;
+        CUDA_TRY(cudaGetLastError());
+        src = dst;
+    }
+    if (o.host) CUDA_TRY(cudaMemcpyAsync(o.user, src, bytes, cudaMemcpyDeviceToHost, st));
     return KG_OK;
 }
 
@@ -243,6 +318,142 @@ static StagedArgs staged_base_args(const kg_hamiltonian *h, const StagedPlan &sp
     return sa;
 }
 
+
+// ---- two-step kernel (kg_tb2.cuh): host-side plan + dispatch ----
+__global__ void kg_tb2_gather_onsite(const double *__restrict__ onsite, const int32_t *__restrict__ hid,
+                                     const int2 *__restrict__ tinfo, int ntiles, int cap1, int cap2,
+                                     double *__restrict__ hons)
+{
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < (int64_t)ntiles * cap1;
+         e += (int64_t)gridDim.x * blockDim.x) {
+        const int t = (int)(e / cap1), j = (int)(e - (int64_t)t * cap1);
+        hons[e] = j < tinfo[t].x ? onsite[hid[(int64_t)t * (cap1 + cap2) + j]] : 0.0;
+    }
+}
+
+// Build the per-tile plan for C columns per site from the packed list (dictionary id << 28 | index,
+// internal order).  Runs once per handle and C, at the first eligible moments call; synchronises.
+static int tb2_build_plan(kg_hamiltonian *h, int C, cudaStream_t st)
+{
+    Tb2Plan &tp = h->tbp[C - 1];
+    tp.built = true;
+    tp.ok = false;
+    if (!h->nlp || h->ndict <= 0 || !kg_tb2_k_supported(h->kmax)) return KG_OK;
+    const int K = h->kmax, KP = tb_kp(K), CS = tb_cs(C);
+    const int64_t n = h->n, ns = h->ns;
+    const int ntiles = (int)((n + CS - 1) / CS);
+    std::vector<int32_t> idx((size_t)ns * K);
+    CUDA_TRY(cudaMemcpyAsync(idx.data(), h->nlp, (size_t)ns * K * 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    // pass 1 and 2 share the marker arrays: mark[m] = tile that last touched m, slot[m] = its local slot
+    std::vector<int32_t> mark((size_t)n, -1), slot((size_t)n, 0);
+    std::vector<int2> tinfo((size_t)ntiles);
+    std::vector<std::vector<int32_t>> halo((size_t)ntiles);    // H1 then H2 ids per tile
+    int max1 = 0, max2 = 0;
+    for (int t = 0; t < ntiles; ++t) {
+        const int64_t s0 = (int64_t)t * CS, s1 = std::min<int64_t>(n, s0 + CS);
+        std::vector<int32_t> &hl = halo[(size_t)t];
+        for (int64_t i = s0; i < s1; ++i)
+            for (int k = 0; k < K; ++k) {
+                const int32_t m = idx[(size_t)k * ns + i] & SG_IDX_MASK;
+                if (m >= s0 && m < s1) continue;
+                if (mark[(size_t)m] != t) { mark[(size_t)m] = t; slot[(size_t)m] = CS + (int)hl.size(); hl.push_back(m); }
+            }
+        const int n1 = (int)hl.size();
+        for (int j = 0; j < n1; ++j) {
+            const int32_t g = hl[(size_t)j];
+            for (int k = 0; k < K; ++k) {
+                const int32_t m = idx[(size_t)k * ns + g] & SG_IDX_MASK;
+                if (m >= s0 && m < s1) continue;
+                if (mark[(size_t)m] != t) { mark[(size_t)m] = t; slot[(size_t)m] = CS + (int)hl.size(); hl.push_back(m); }
+            }
+        }
+        const int n2 = (int)hl.size() - n1;
+        tinfo[(size_t)t] = make_int2(n1, n2);
+        max1 = std::max(max1, n1); max2 = std::max(max2, n2);
+    }
+    const int cap1 = std::max(8, (max1 + 7) / 8 * 8), cap2 = std::max(8, (max2 + 7) / 8 * 8);
+    if (CS + cap1 + cap2 > TB_SLOT_MASK + 1 || TB_HEADER + 2 * tb_stage_bytes(C, K, cap1, cap2) > (size_t)227 * 1024) return KG_OK;
+    // pass 2: tile-local rows (own rows, then H1 rows)
+    const size_t rstride = (size_t)(CS + cap1) * KP;
+    std::vector<uint16_t> rows((size_t)ntiles * rstride, 0);
+    std::vector<int32_t> hid((size_t)ntiles * (cap1 + cap2), 0);
+    for (int t = 0; t < ntiles; ++t) {
+        const int64_t s0 = (int64_t)t * CS, s1 = std::min<int64_t>(n, s0 + CS);
+        const std::vector<int32_t> &hl = halo[(size_t)t];
+        const int n1 = tinfo[(size_t)t].x;
+        for (size_t j = 0; j < hl.size(); ++j) {
+            mark[(size_t)hl[j]] = t; slot[(size_t)hl[j]] = CS + (int)j;
+            hid[(size_t)t * (cap1 + cap2) + j] = hl[j];
+        }
+        uint16_t *rt = rows.data() + (size_t)t * rstride;
+        auto fill = [&](int row, int64_t site) {
+            for (int k = 0; k < K; ++k) {
+                const uint32_t w = (uint32_t)idx[(size_t)k * ns + site];
+                const int32_t m = (int32_t)(w & SG_IDX_MASK);
+                const int sl = (m >= s0 && m < s1) ? (int)(m - s0) : slot[(size_t)m];
+                rt[(size_t)row * KP + k] = (uint16_t)(((w >> 28) << 12) | (uint32_t)sl);
+            }
+            for (int k = K; k < KP; ++k) rt[(size_t)row * KP + k] = (uint16_t)row;      // unused: id 0 (value 0)
+        };
+        for (int64_t i = s0; i < s1; ++i) fill((int)(i - s0), i);
+        for (int j = 0; j < n1; ++j) fill(CS + j, hl[(size_t)j]);
+    }
+    cudaError_t e;
+    if ((e = cudaMalloc(&tp.tinfo, (size_t)ntiles * sizeof(int2))) != cudaSuccess ||
+        (e = cudaMalloc(&tp.rows, rows.size() * 2)) != cudaSuccess || (e = cudaMalloc(&tp.hid, hid.size() * 4)) != cudaSuccess ||
+        (e = cudaMalloc(&tp.hons, (size_t)ntiles * cap1 * 8)) != cudaSuccess)
+        return fail(KG_ENOMEM, "two-step plan allocation: %s", cudaGetErrorString(e));
+    tp.bytes = (size_t)ntiles * sizeof(int2) + rows.size() * 2 + hid.size() * 4 + (size_t)ntiles * cap1 * 8;
+    CUDA_TRY(cudaMemcpyAsync(tp.tinfo, tinfo.data(), (size_t)ntiles * sizeof(int2), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(tp.rows, rows.data(), rows.size() * 2, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(tp.hid, hid.data(), hid.size() * 4, cudaMemcpyHostToDevice, st));
+    kg_tb2_gather_onsite<<<std::min<int64_t>(((int64_t)ntiles * cap1 + 255) / 256, (int64_t)h->num_sms * 8), 256, 0, st>>>(
+        h->onsite, tp.hid, tp.tinfo, ntiles, cap1, cap2, tp.hons);
+    h->launches++;
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaStreamSynchronize(st));             // the host vectors go out of scope
+    tp.cap1 = cap1; tp.cap2 = cap2; tp.ntiles = ntiles;
+    tp.ok = true;
+    return KG_OK;
+}
+
+struct Tb2Launch { bool ok; int grid, nst; size_t smem; };
+
+// Is the two-step kernel to be used for a doubling moment loop on C contiguous columns?
+static int tb2_plan(kg_hamiltonian *h, int mode, int C, cudaStream_t st, Tb2Launch *out)
+{
+    out->ok = false;
+    if (h->tb2 == 0 || !h->staged || !h->doubling || C > 2 || (mode == MODE_MOMX && C != 2) ||
+        (mode != MODE_MOM2 && mode != MODE_MOMX))
+        return KG_OK;
+    const int64_t nt = (h->n + tb_cs(C) - 1) / tb_cs(C);
+    if (h->tb2 < 0 && (!h->perm || nt < 4 * (int64_t)h->num_sms)) return KG_OK;    // auto: re-ordered sites, >= 4 tiles per SM
+    Tb2Plan &tp = h->tbp[C - 1];
+    if (!tp.built) { int rc = tb2_build_plan(h, C, st); if (rc) return rc; }
+    if (!tp.ok) return KG_OK;
+    // one persistent CTA per SM; as many shared-memory stages as fit (2..4)
+    const size_t stage = tb_stage_bytes(C, h->kmax, tp.cap1, tp.cap2);
+    out->nst = (int)std::min<size_t>(h->stages > 0 ? (size_t)h->stages : (size_t)3, ((size_t)227 * 1024 - TB_HEADER) / stage);
+    if (out->nst > TB_MAX_STAGES) out->nst = TB_MAX_STAGES;
+    if (out->nst < 2) return KG_OK;
+    out->smem = TB_HEADER + (size_t)out->nst * stage;
+    out->grid = (int)std::min<int64_t>(tp.ntiles, (int64_t)h->num_sms);
+    out->ok = true;
+    return KG_OK;
+}
+
+static Tb2Args tb2_base_args(const kg_hamiltonian *h, int C)
+{
+    const Tb2Plan &tp = h->tbp[C - 1];
+    Tb2Args a;
+    memset(&a, 0, sizeof(a));
+    a.tinfo = tp.tinfo; a.rows = tp.rows; a.hid = tp.hid; a.hons = tp.hons; a.onsite = h->onsite;
+    memcpy(a.dict, h->dict, sizeof(a.dict));
+    a.n = h->n; a.cap1 = tp.cap1; a.cap2 = tp.cap2; a.ntiles = tp.ntiles;
+    return a;
+}
+
 static bool r_ok(int R, bool allow16) { return R == 1 || R == 2 || R == 4 || R == 8 || (allow16 && R == 16); }
 
 // --------------------------------------------------------------------------------------
@@ -329,6 +540,8 @@ static int create_from_device_list(kg_hamiltonian **out, int64_t n, int kmax, co
     h->n = n; h->ns = (n + SG_TILE_E - 1) / SG_TILE_E * SG_TILE_E; h->kmax = kmax;
     h->s = s; h->e0 = e0; h->period = period;
     h->nl = h->nlp = nullptr; h->hop = h->xhop = h->onsite = nullptr;
+    h->perm = h->iperm = nullptr;
+    h->tb2 = -1; memset(h->tbp, 0, sizeof(h->tbp));
     h->ndict = 0; h->staged = 1; h->stages = 0; h->staged_ctas = 0; h->alternate = 1; h->doubling = 1; h->clenshaw = 1; h->pdl = -1;
     memset(h->dict, 0, sizeof(h->dict));
     memset(h->ws, 0, sizeof(h->ws));
@@ -350,9 +563,27 @@ static int create_from_device_list(kg_hamiltonian **out, int64_t n, int kmax, co
         return cleanup(fail(KG_ENOMEM, "matrix allocation: %s", cudaGetErrorString(e)));
     if ((e = cudaMemsetAsync(d_flags, 0, 16, st)) != cudaSuccess)
         return cleanup(fail(KG_ECUDA, "memset: %s", cudaGetErrorString(e)));
+    // site re-ordering: recursive breadth-first bisection of the neighbour list on the host
+    // (kg_partition.h), so that every aligned block of consecutive internal sites is a compact patch
+    if (g_reorder > 0 || (g_reorder < 0 && n >= KG_REORDER_MIN_SITES)) {
+        std::vector<int32_t> h_nn((size_t)n), h_nl((size_t)n * kmax), perm, iperm((size_t)n);
+        if ((e = cudaMemcpyAsync(h_nn.data(), d_nn, (size_t)n * 4, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+            (e = cudaMemcpyAsync(h_nl.data(), d_nl, (size_t)n * kmax * 4, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+            (e = cudaStreamSynchronize(st)) != cudaSuccess)
+            return cleanup(fail(KG_ECUDA, "neighbour list to host: %s", cudaGetErrorString(e)));
+        kg_partition_host(n, kmax, h_nn.data(), h_nl.data(), KG_REORDER_LEAF, perm);
+        for (int64_t i = 0; i < n; ++i) iperm[(size_t)perm[(size_t)i]] = (int32_t)i;
+        if ((e = cudaMalloc(&h->perm, (size_t)n * 4)) != cudaSuccess || (e = cudaMalloc(&h->iperm, (size_t)n * 4)) != cudaSuccess)
+            return cleanup(fail(KG_ENOMEM, "permutation allocation: %s", cudaGetErrorString(e)));
+        h->matrix_bytes += (size_t)n * 8;
+        if ((e = cudaMemcpyAsync(h->perm, perm.data(), (size_t)n * 4, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+            (e = cudaMemcpyAsync(h->iperm, iperm.data(), (size_t)n * 4, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+            (e = cudaStreamSynchronize(st)) != cudaSuccess)          // the host vectors go out of scope
+            return cleanup(fail(KG_ECUDA, "permutation upload: %s", cudaGetErrorString(e)));
+    }
     const int grid = (int)std::min<int64_t>((h->ns + 255) / 256, (int64_t)h->num_sms * 8);
     kg_build_matrix<<<grid, 256, 0, st>>>(n, h->ns, kmax, d_nn, d_nl, d_hop, d_ons, d_x, period, e0, s,
-                                          h->nl, h->hop, h->xhop, h->onsite, d_flags,
+                                          h->perm, h->iperm, h->nl, h->hop, h->xhop, h->onsite, d_flags,
                                           (unsigned long long *)(d_flags + 2));
     h->launches++;
     unsigned int host_flags[4];
@@ -512,6 +743,8 @@ extern "C" int kg_destroy_hamiltonian(kg_hamiltonian *h)
     if (!h) return KG_OK;
     for (auto &g : h->graphs) cudaGraphExecDestroy(g.exec);
     cudaFree(h->nl); cudaFree(h->nlp); cudaFree(h->hop); cudaFree(h->xhop); cudaFree(h->onsite);
+    cudaFree(h->perm); cudaFree(h->iperm);
+    for (auto &tp : h->tbp) { cudaFree(tp.tinfo); cudaFree(tp.rows); cudaFree(tp.hid); cudaFree(tp.hons); }
     for (int i = 0; i < WS_COUNT; ++i) cudaFree(h->ws[i]);
     delete h;
     return KG_OK;
@@ -520,7 +753,7 @@ extern "C" int kg_destroy_hamiltonian(kg_hamiltonian *h)
 extern "C" size_t kg_workspace_bytes(const kg_hamiltonian *h)
 {
     if (!h) return 0;
-    size_t t = h->matrix_bytes;
+    size_t t = h->matrix_bytes + h->tbp[0].bytes + h->tbp[1].bytes;
     for (int i = 0; i < WS_COUNT; ++i) t += h->ws_bytes[i];
     return t;
 }
@@ -550,6 +783,7 @@ extern "C" int kg_set_option(kg_hamiltonian *h, int option, int64_t value)
     case KG_OPT_DOUBLING: h->doubling = value != 0; break;
     case KG_OPT_CLENSHAW: h->clenshaw = value != 0; break;
     case KG_OPT_PDL: h->pdl = value < 0 ? -1 : (value != 0); break;
+    case KG_OPT_TWO_STEP: h->tb2 = value < 0 ? -1 : (value != 0); break;
     case KG_OPT_DICT:
         if (value != 0) return fail(KG_EINVAL, "the dictionary can only be switched off");
         h->ndict = 0; break;
@@ -623,13 +857,58 @@ static int moments_device(kg_hamiltonian *h, const c128 *phiL, int ldL, const c1
     const int mode = cross ? MODE_MOMX : dbl ? MODE_MOM2 : MODE_MOM;
     const int PR = cross ? R / 2 : R;                        // columns of a partial row / rows of mu
     const StagedPlan sp = staged_plan(h, mode, R);
-    const int grid = sp.ok ? sp.grid : grid_for(h, elems);   // one partial row shape for both kernels
-    void *ta, *tb, *part;
     int rc;
+    // two Chebyshev steps per pass (kg_tb2.cuh) when the vectors are contiguous [n][R], R <= 2
+    Tb2Launch tl;
+    tl.ok = false;
+    if (dbl && ldL == R && ldR == R && M / 2 >= 3 && (rc = tb2_plan(h, mode, R, st, &tl))) return rc;
+    const int grid = tl.ok ? tl.grid : sp.ok ? sp.grid : grid_for(h, elems);   // one partial row shape for all kernels of the call
+    void *ta, *tb, *part;
     if ((rc = ws_get(h, WS_TA, (size_t)elems * 16, &ta)) || (rc = ws_get(h, WS_TB, (size_t)elems * 16, &tb)) ||
         (rc = ws_get(h, WS_PART, (size_t)(M + 1) * grid * R * 16, &part)))
         return rc;
-    if (want_graph(h, elems, st)) {
+    if (tl.ok) {
+        void *tc, *td;
+        if ((rc = ws_get(h, WS_TC, (size_t)elems * 16, &tc)) || (rc = ws_get(h, WS_TD, (size_t)elems * 16, &td))) return rc;
+        const size_t prow = (size_t)grid * PR;
+        c128 *P = (c128 *)part;
+        // m = 1: T_1 = H~ T_0 and the partials of moments 0, 1, 2 (one-thread-per-element kernel)
+        StepArgs a = base_args(h);
+        a.phiL = phiL; a.ld_L = ldL; a.alpha = 1.0;
+        a.cur = phiR; a.ld_cur = ldR; a.next = (c128 *)ta;
+        a.partial0 = P; a.partial = P + prow; a.partial2 = P + 2 * prow;
+        CUDA_TRY(launch_step(h, mode, true, R, a, grid, st));
+        // steps m = 2 .. M/2 in pairs; step m makes T_m and the partials of moments 2m - 1 and 2m
+        Tb2Args ta2 = tb2_base_args(h, R);
+        ta2.nstages = tl.nst;
+        const c128 *prev = phiR, *cur = (const c128 *)ta;
+        std::vector<c128 *> freeb = {(c128 *)tb, (c128 *)tc, (c128 *)td};
+        const int m_end = M / 2 + 1;
+        int pass = 0;
+        for (int m = 2; m < m_end; ++pass) {
+            const int nstep = (m + 1 < m_end) ? 2 : 1;
+            ta2.cur = cur; ta2.prev = prev;
+            ta2.next1 = freeb[0]; ta2.next2 = nstep == 2 ? freeb[1] : nullptr;
+            ta2.p1 = P + (size_t)(2 * m - 1) * prow; ta2.p2 = P + (size_t)(2 * m) * prow;
+            ta2.p3 = P + (size_t)(2 * m + 1) * prow; ta2.p4 = P + (size_t)(2 * m + 2) * prow;
+            ta2.reverse = h->alternate ? (pass & 1) : 0;
+            h->launches++;
+            CUDA_TRY(kg_tb2_launch(h->kmax, mode, R, h->has_onsite, nstep, ta2, grid, tl.smem, h->device, st));
+            // rotate: the two oldest vectors become free (the caller's phiR is never written)
+            c128 *old_prev = const_cast<c128 *>(prev), *old_cur = const_cast<c128 *>(cur);
+            if (nstep == 2) {
+                prev = freeb[0]; cur = freeb[1];
+                freeb.erase(freeb.begin(), freeb.begin() + 2);
+                if (old_prev != phiR) freeb.push_back(old_prev);
+                freeb.push_back(old_cur);
+            } else {
+                prev = cur; cur = freeb[0];
+                freeb.erase(freeb.begin());
+                if (old_prev != phiR) freeb.push_back(old_prev);
+            }
+            m += nstep;
+        }
+    } else if (want_graph(h, elems, st)) {
         cudaGraphExec_t exec = nullptr;
         for (auto &g : h->graphs)
             if (g.phiL == phiL && g.phiR == phiR && g.ldL == ldL && g.ldR == ldR && g.R == R && g.M == M &&
@@ -847,12 +1126,11 @@ extern "C" int kg_moments(kg_hamiltonian *h, const kg_c128 *phiL, const kg_c128 
     if (!r_ok(R, false)) return fail(KG_EUNSUPPORTED, "R must be 1, 2, 4 or 8");
     if (M < 2) return fail(KG_EINVAL, "M must be >= 2");
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t vbytes = (size_t)h->n * R * 16;
     const void *dL, *dR;
     int rc;
-    if ((rc = stage_in(h, WS_IN0, phiL, vbytes, st, &dL))) return rc;
+    if ((rc = vec_in(h, WS_IN0, phiL, R, st, &dL))) return rc;
     if (phiR == phiL) dR = dL;
-    else if ((rc = stage_in(h, WS_IN1, phiR, vbytes, st, &dR))) return rc;
+    else if ((rc = vec_in(h, WS_IN1, phiR, R, st, &dR))) return rc;
     OutStage o;
     if ((rc = stage_out(h, WS_MU, mu, (size_t)R * M * 16, &o))) return rc;
     if ((rc = moments_device(h, (const c128 *)dL, R, (const c128 *)dR, R, R, M, (c128 *)o.dev, M, st))) return rc;
@@ -872,13 +1150,12 @@ extern "C" int kg_evolve(kg_hamiltonian *h, const kg_c128 *in, kg_c128 *out, int
     if (!r_ok(R, true)) return fail(KG_EUNSUPPORTED, "R must be 1, 2, 4, 8 or 16");
     if (dt_fs == 0.0 || !std::isfinite(dt_fs)) return fail(KG_EINVAL, "dt_fs must be finite and non-zero");
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t vbytes = (size_t)h->n * R * 16;
     const void *din;
-    OutStage o;
+    VecOut o;
     int rc;
-    if ((rc = stage_in(h, WS_IN0, in, vbytes, st, &din)) || (rc = stage_out(h, WS_OUT0, out, vbytes, &o))) return rc;
+    if ((rc = vec_in(h, WS_IN0, in, R, st, &din)) || (rc = vec_out(h, WS_OUT0, out, R, &o))) return rc;
     if ((rc = evolve_device(h, (const c128 *)din, R, (c128 *)o.dev, R, dt_fs, bessel_eps, st))) return rc;
-    return finish_out(o, st);
+    return vec_out_finish(h, o, st);
 }
 
 extern "C" int kg_apply_velocity(kg_hamiltonian *h, const kg_c128 *in, kg_c128 *out, int R, void *stream)
@@ -887,13 +1164,12 @@ extern "C" int kg_apply_velocity(kg_hamiltonian *h, const kg_c128 *in, kg_c128 *
     if (in == out) return fail(KG_EINVAL, "kg_apply_velocity: out must not alias in");
     if (!r_ok(R, true)) return fail(KG_EUNSUPPORTED, "R must be 1, 2, 4, 8 or 16");
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t vbytes = (size_t)h->n * R * 16;
     const void *din;
-    OutStage o;
+    VecOut o;
     int rc;
-    if ((rc = stage_in(h, WS_IN0, in, vbytes, st, &din)) || (rc = stage_out(h, WS_OUT0, out, vbytes, &o))) return rc;
+    if ((rc = vec_in(h, WS_IN0, in, R, st, &din)) || (rc = vec_out(h, WS_OUT0, out, R, &o))) return rc;
     if ((rc = velocity_device(h, (const c128 *)din, R, (c128 *)o.dev, R, R, st))) return rc;
-    return finish_out(o, st);
+    return vec_out_finish(h, o, st);
 }
 
 extern "C" int kg_evolve_x(kg_hamiltonian *h, kg_c128 *psi, kg_c128 *psix, int R, double dt_fs,
@@ -908,13 +1184,26 @@ extern "C" int kg_evolve_x(kg_hamiltonian *h, kg_c128 *psi, kg_c128 *psix, int R
     const void *dpsi, *dpsix;
     void *o0, *o1;
     int rc;
-    if ((rc = stage_in(h, WS_IN0, psi, vbytes, st, &dpsi)) || (rc = stage_in(h, WS_IN1, psix, vbytes, st, &dpsix)) ||
+    if ((rc = vec_in(h, WS_IN0, psi, R, st, &dpsi)) || (rc = vec_in(h, WS_IN1, psix, R, st, &dpsix)) ||
         (rc = ws_get(h, WS_OUT0, vbytes, &o0)) || (rc = ws_get(h, WS_OUT1, vbytes, &o1)))
         return rc;
     if ((rc = pair_device(h, (const c128 *)dpsi, (const c128 *)dpsix, (c128 *)o0, (c128 *)o1, R, dt_fs, bessel_eps, st)))
         return rc;
-    CUDA_TRY(cudaMemcpyAsync(psi, o0, vbytes, cudaMemcpyDefault, st));
-    CUDA_TRY(cudaMemcpyAsync(psix, o1, vbytes, cudaMemcpyDefault, st));
+    // back into the caller's arrays (in place for the caller): inverse permutation and / or copy
+    void *user[2] = {psi, psix}, *res[2] = {o0, o1};
+    for (int q = 0; q < 2; ++q) {
+        const bool on_dev = is_device_ptr(user[q]);
+        const void *src = res[q];
+        if (h->perm) {
+            void *dst = user[q];
+            if (!on_dev && (rc = ws_get(h, WS_RAW0 + q, vbytes, &dst))) return rc;
+            kg_permute_rows<<<grid_for(h, h->n * R), 256, 0, st>>>((const c128 *)res[q], (c128 *)dst, h->iperm, h->n, R);
+            h->launches++;
+            CUDA_TRY(cudaGetLastError());
+            src = dst;
+        }
+        if (src != user[q]) CUDA_TRY(cudaMemcpyAsync(user[q], src, vbytes, cudaMemcpyDefault, st));
+    }
     return KG_OK;
 }
 
@@ -939,7 +1228,7 @@ extern "C" int kg_vac(kg_hamiltonian *h, const kg_c128 *phi, int R, int M, int n
     const void *dphi;
     void *s0, *s1, *pl;
     OutStage o;
-    if ((rc = stage_in(h, WS_IN0, phi, vbytes, st, &dphi)) || (rc = ws_get(h, WS_S0, 2 * vbytes, &s0)) ||
+    if ((rc = vec_in(h, WS_IN0, phi, R, st, &dphi)) || (rc = ws_get(h, WS_S0, 2 * vbytes, &s0)) ||
         (rc = ws_get(h, WS_S1, 2 * vbytes, &s1)) || (rc = ws_get(h, WS_PHIL, 2 * vbytes, &pl)) ||
         (rc = stage_out(h, WS_MU, mu, (size_t)R * (n_steps + 1) * M * 16, &o)))
         return rc;
@@ -978,7 +1267,7 @@ extern "C" int kg_msd(kg_hamiltonian *h, const kg_c128 *phi, int R, int M, int n
     const void *dphi;
     void *p0, *p1, *x0, *x1;
     OutStage o;
-    if ((rc = stage_in(h, WS_IN0, phi, vbytes, st, &dphi)) || (rc = ws_get(h, WS_S0, vbytes, &p0)) ||
+    if ((rc = vec_in(h, WS_IN0, phi, R, st, &dphi)) || (rc = ws_get(h, WS_S0, vbytes, &p0)) ||
         (rc = ws_get(h, WS_S1, vbytes, &p1)) || (rc = ws_get(h, WS_X0, vbytes, &x0)) ||
         (rc = ws_get(h, WS_X1, vbytes, &x1)) ||
         (rc = stage_out(h, WS_MU, mu, (size_t)R * (n_steps + 1) * M * 16, &o)))
@@ -987,8 +1276,10 @@ extern "C" int kg_msd(kg_hamiltonian *h, const kg_c128 *phi, int R, int M, int n
     CUDA_TRY(cudaMemcpyAsync(P, dphi, vbytes, cudaMemcpyDeviceToDevice, st));   // psi_0 = phi
     CUDA_TRY(cudaMemsetAsync(X, 0, vbytes, st));                                // psix_0 = 0
     const int64_t rstride = (int64_t)(n_steps + 1) * M;
+    // row k = 0: psix_0 = 0, so C_m^MSD(0) = 0 exactly (eq 44 starts from zero) — written, not computed
+    CUDA_TRY(cudaMemset2DAsync(o.dev, (size_t)rstride * 16, 0, (size_t)M * 16, (size_t)R, st));
     for (int k = 0; k <= n_steps; ++k) {
-        if ((rc = moments_device(h, X, R, X, R, R, M, (c128 *)o.dev + (size_t)k * M, rstride, st))) return rc;
+        if (k > 0 && (rc = moments_device(h, X, R, X, R, R, M, (c128 *)o.dev + (size_t)k * M, rstride, st))) return rc;
         if (k == n_steps) break;
         if ((rc = pair_device(h, P, X, Pn, Xn, R, dt_fs, bessel_eps, st))) return rc;
         c128 *t = P; P = Pn; Pn = t;
@@ -1107,9 +1398,9 @@ extern "C" int kg_fourier_moments(kg_hamiltonian *h, const kg_c128 *phiL, const 
     void *b0, *b1, *part;
     OutStage o;
     int rc;
-    if ((rc = stage_in(h, WS_IN0, phiL, vbytes, st, &dL))) return rc;
+    if ((rc = vec_in(h, WS_IN0, phiL, R, st, &dL))) return rc;
     if (phiR == phiL) dR = dL;
-    else if ((rc = stage_in(h, WS_IN1, phiR, vbytes, st, &dR))) return rc;
+    else if ((rc = vec_in(h, WS_IN1, phiR, R, st, &dR))) return rc;
     if ((rc = ws_get(h, WS_S0, vbytes, &b0)) || (rc = ws_get(h, WS_S1, vbytes, &b1)) ||
         (rc = ws_get(h, WS_PART, (size_t)rows * grid * R * 16, &part)) ||
         (rc = stage_out(h, WS_MU, F, (size_t)R * rows * 16, &o)))

@@ -196,11 +196,14 @@ __global__ void kg_copy_cols(const c128 *__restrict__ src, int ld_src, c128 *__r
 __global__ void kg_build_matrix(int64_t n, int64_t ns, int kmax, const int32_t *__restrict__ nn,
                                 const int32_t *__restrict__ nl_in, const double *__restrict__ hop_in,
                                 const double *__restrict__ onsite_in, const double *__restrict__ x,
-                                double period, double e0, double s, int32_t *__restrict__ nl,
+                                double period, double e0, double s, const int32_t *__restrict__ perm,
+                                const int32_t *__restrict__ iperm, int32_t *__restrict__ nl,
                                 double *__restrict__ hop, double *__restrict__ xhop,
                                 double *__restrict__ onsite, unsigned int *flags,
                                 unsigned long long *gersh)
 {
+    // perm / iperm (may be NULL): internal row i is the caller's row perm[i]; the caller's site m is
+    // internal site iperm[m] (site re-ordering, kg_partition.h)
     unsigned int bad = 0;
     double gmax = 0.0;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < ns;
@@ -210,11 +213,12 @@ __global__ void kg_build_matrix(int64_t n, int64_t ns, int kmax, const int32_t *
             onsite[i] = 0.0;
             continue;
         }
-        int cnt = nn[i];
+        const int64_t io = perm ? perm[i] : i;              // the caller's index of this row
+        int cnt = nn[io];
         if (cnt < 0 || cnt > kmax) { bad |= 2u; cnt = 0; }
-        const double xi = x[i];
+        const double xi = x[io];
         if (!isfinite(xi)) bad |= 4u;
-        const double eps = onsite_in ? onsite_in[i] : 0.0;
+        const double eps = onsite_in ? onsite_in[io] : 0.0;
         if (!isfinite(eps)) bad |= 4u;
         double g = fabs(eps - e0);
         onsite[i] = (eps - e0) / s;
@@ -222,27 +226,28 @@ __global__ void kg_build_matrix(int64_t n, int64_t ns, int kmax, const int32_t *
             int32_t m = (int32_t)i;
             double h = 0.0, w = 0.0;
             if (k < cnt) {
-                m = nl_in[k * n + i];
-                h = hop_in[k * n + i];
-                if (m < 0 || m >= n) { bad |= 1u; m = (int32_t)i; h = 0.0; }
+                int32_t mo = nl_in[k * n + io];
+                h = hop_in[k * n + io];
+                if (mo < 0 || mo >= n) { bad |= 1u; mo = (int32_t)io; h = 0.0; }
                 if (!isfinite(h)) { bad |= 4u; h = 0.0; }
-                double d = x[m] - xi;                       // Delta = X_m - X_i, minimum image
+                double d = x[mo] - xi;                      // Delta = X_m - X_i, minimum image
                 if (period > 0.0) {
                     if (d > 0.5 * period) d -= period;
                     if (d < -0.5 * period) d += period;
                 }
                 w = (-d) * h / s;                           // (X_i - X_m) H_im / s
                 g += fabs(h);
-                if (m != i) {                               // symmetry: H_mi must equal H_im
+                if (mo != io) {                             // symmetry: H_mi must equal H_im
                     bool found = false;
-                    int cm = nn[m];
+                    int cm = nn[mo];
                     if (cm < 0 || cm > kmax) cm = 0;
                     for (int q = 0; q < cm; ++q)
-                        if (nl_in[q * n + m] == (int32_t)i && hop_in[q * n + m] == h) found = true;
+                        if (nl_in[q * n + mo] == (int32_t)io && hop_in[q * n + mo] == h) found = true;
                     if (!found) bad |= 8u;
                 } else {
                     bad |= 8u;                              // diagonal belongs in onsite_eV
                 }
+                m = iperm ? iperm[mo] : mo;
             }
             nl[k * ns + i] = m;
             hop[k * ns + i] = h / s;
@@ -252,6 +257,20 @@ __global__ void kg_build_matrix(int64_t n, int64_t ns, int kmax, const int32_t *
     }
     if (bad) atomicOr(flags, bad);
     atomicMax(gersh, (unsigned long long)__double_as_longlong(gmax));
+}
+
+// dst[i*R + r] = src[map[i]*R + r]: caller order -> internal order with map = perm, and back with
+// map = iperm (one thread per element, coalesced writes, 16-byte gathers)
+__global__ void kg_permute_rows(const c128 *__restrict__ src, c128 *__restrict__ dst,
+                                const int32_t *__restrict__ map, int64_t n, int R)
+{
+    const int64_t total = n * R;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total;
+         e += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t i = e / R;
+        const int r = (int)(e - i * R);
+        dst[e] = src[(int64_t)map[i] * R + r];
+    }
 }
 
 // CSR -> k-major list (rows become columns of the ELL slabs)
