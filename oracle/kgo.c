@@ -166,6 +166,27 @@ int64_t kgo_compact(int64_t n_full, const uint8_t *vacant, const double *x, cons
     return c;
 }
 
+/* Zigzag graphene nanoribbon (Fig. 4: "ZGNR 65536 x 16"): N_y zigzag chains   */
+/* (P:91-93), periodic along x (the zigzag direction, the transport axis), zigzag edges.  Cut    */
+/* from a sheet of ncx x (N_y/2 + 1) cells that is open along y: the sheet's open edges are      */
+/* "bearded" (the b0 sites of the bottom cell row and the b3 sites of the top one hang on one    */
+/* bond), a zigzag edge is obtained by removing the bottom row's b0 sites and the top row's      */
+/* b1, b2, b3 sites — the cut then runs through the vertical bonds, every edge site keeps two    */
+/* neighbours, and the N_y chains are {b1,b2} of cell rows 0..N_y/2-1 and {b3 of row c, b0 of    */
+/* row c+1}, c = 0..N_y/2-1.  Writes vacant[4 ncx (N_y/2+1)] for kgo_compact; N_y must be even.  */
+int kgo_zgnr_mask(int64_t ncx, int64_t n_chains, uint8_t *vacant)
+{
+    if (n_chains < 2 || (n_chains & 1)) return 1;
+    const int64_t ncy = n_chains / 2 + 1;
+    for (int64_t cy = 0; cy < ncy; ++cy)
+        for (int64_t cx = 0; cx < ncx; ++cx)
+            for (int b = 0; b < 4; ++b) {
+                const int64_t i = 4 * (cy * ncx + cx) + b;
+                vacant[i] = (uint8_t)((cy == 0 && b == 0) || (cy == ncy - 1 && b != 0));
+            }
+    return 0;
+}
+
 /* Anderson on-site energies (BASELINE config 4; reading g17):                 */
 /* eps_j = W * (u(seed, stream 1, j) - 0.5).                                   */
 void kgo_anderson(int64_t n, double w_eV, uint64_t seed, double *eps)

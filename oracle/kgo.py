@@ -122,6 +122,16 @@ def remove_sites(lat: Lattice, vacant, t_eV=-2.7):
     return Lattice(n_out, 3, nn, nl, hop_from_nn(nn, t_eV), None, x, y, lat.period_x, lat.period_y)
 
 
+def zgnr(ncx, n_chains, a_nm=0.142, t_eV=-2.7):
+    """Zigzag ribbon of n_chains zigzag chains (even), ncx cells (2 ncx dimer lines) long, periodic
+    along x: kgo_honeycomb (open along y) + kgo_zgnr_mask + kgo_compact."""
+    sheet = honeycomb(ncx, n_chains // 2 + 1, periodic_x=True, periodic_y=False, a_nm=a_nm, t_eV=t_eV)
+    vac = np.zeros(sheet.n, np.uint8)
+    rc = lib().kgo_zgnr_mask(C.c_int64(ncx), C.c_int64(n_chains), _p(vac))
+    assert rc == 0
+    return remove_sites(sheet, vac, t_eV)
+
+
 def anderson(n, w_eV, seed):
     eps = np.empty(n)
     lib().kgo_anderson(C.c_int64(n), C.c_double(w_eV), C.c_uint64(seed), _p(eps))

@@ -153,6 +153,24 @@ def remove_sites(lat: Lattice, vacant: np.ndarray, t_eV=T_EV) -> Lattice:
                    lat.y[old].copy(), lat.period_x, lat.period_y, dict(lat.meta))
 
 
+def zgnr(ncx: int, n_chains: int, a_nm=A_NM, t_eV=T_EV) -> Lattice:
+    """Zigzag graphene nanoribbon (the paper's ballistic test system, Fig. 4: "65536 x 16"):
+    n_chains zigzag chains (even; the paper's N_y), ncx cells = 2 ncx dimer lines (N_x) long, periodic
+    along x (zigzag direction = transport axis).  Cut from a sheet of ncx x (n_chains/2 + 1) cells open
+    along y by removing the bottom cell row's b0 sites and the top row's b1, b2, b3 sites: the cut runs
+    through the vertical bonds, so both edges are zigzag and every edge site keeps two neighbours
+    (the open sheet itself has "bearded" edges: sites hanging on one bond)."""
+    assert n_chains >= 2 and n_chains % 2 == 0
+    ncy = n_chains // 2 + 1
+    sheet = honeycomb(ncx, ncy, periodic_x=True, periodic_y=False, a_nm=a_nm, t_eV=t_eV)
+    site = np.arange(sheet.n, dtype=np.int64)
+    b, cy = site & 3, (site >> 2) // ncx
+    vacant = (((cy == 0) & (b == 0)) | ((cy == ncy - 1) & (b != 0))).astype(np.uint8)
+    lat = remove_sites(sheet, vacant, t_eV)
+    lat.meta.update({"n_chains": n_chains, "width_nm": (1.5 * n_chains - 1.0) * a_nm})
+    return lat
+
+
 def anderson(n: int, w_eV: float, seed: int) -> np.ndarray:
     """eps_j = W (u(seed, 1, j) - 1/2)."""
     return w_eV * (uniform(seed, 1, np.arange(n, dtype=np.uint64)) - 0.5)
@@ -221,7 +239,13 @@ def make_config(idx: int, shrink: int = 1) -> Config:
         lat = remove_sites(full, vac)
         return Config("c5_batched_2000x2000", lat, lat.x, lat.period_x, 3 * t * 1.05, 0.0,
                       8, 3000, 50, _dt(8), 3, 1001)
-    raise ValueError("config index must be 1..5")
+    if idx == 6:
+        # the paper's own ballistic system (Fig. 4): ZGNR with N_x = 65536 dimer lines
+        # (32768 cells) and N_y = 16 zigzag chains = 1 048 576 sites; Einstein MSD, transport along x
+        lat = zgnr(32768 // shrink, 16)
+        return Config("zgnr_65536x16", lat, lat.x, lat.period_x, 3 * t * 1.05, 0.0,
+                      1, 2000, 400, _dt(1), 0, 1001)
+    raise ValueError("config index must be 1..6 (6 = the paper's ZGNR 65536 x 16)")
 
 
 def energy_grid(n_energies: int) -> np.ndarray:

@@ -147,3 +147,37 @@ def test_make_config_small():
     assert c3.lattice.n == 15 * 200 * 4 and c3.period == c3.lattice.period_y
     c4 = W.make_config(4, shrink=50)
     assert abs(c4.scale - 9.9225) < 1e-12 and c4.lattice.onsite is not None
+
+
+@pytest.mark.parametrize("ncx,chains", [(7, 4), (16, 16), (5, 2)])
+def test_zgnr_bit_exact_and_zigzag_edges(kgo, ncx, chains):
+    """Zigzag ribbon (the paper's Fig. 4 system, "65536 x 16"): the two independent generators
+    agree bit for bit; N = N_x N_y sites (N_x = 2 ncx dimer lines, N_y chains); both edges are
+    zigzag — no site hangs on one bond (the open sheet's bearded edge), the 2 ncx sites of the outermost
+    y rows have exactly two neighbours, every other site three; bipartite; the cut runs through the
+    vertical bonds (width (3 N_y / 2 - 1) a)."""
+    a, b = kgo.zgnr(ncx, chains), W.zgnr(ncx, chains)
+    assert a.n == b.n == 2 * ncx * chains
+    for f in ("nn", "nl", "hop", "x", "y"):
+        assert np.array_equal(getattr(a, f), getattr(b, f)), f
+    assert a.period_x == b.period_x and b.period_y == 0.0
+    assert set(np.unique(b.nn)) <= {2, 3} and b.nn.min() >= 2
+    edge = (b.y == b.y.min()) | (b.y == b.y.max())
+    assert edge.sum() == 2 * ncx and np.all(b.nn[edge] == 2) and np.all(b.nn[~edge] == 3)
+    assert abs((b.y.max() - b.y.min()) - (1.5 * chains - 1.0) * 0.142) < 1e-12
+    nl = b.nl.reshape(3, b.n)
+    i = np.broadcast_to(np.arange(b.n), (3, b.n))
+    valid = np.arange(3)[:, None] < b.nn[None, :]
+    dx = b.x[nl] - b.x[i]
+    dx -= b.period_x * np.round(dx / b.period_x)
+    bond = np.hypot(dx, b.y[nl] - b.y[i])[valid]
+    assert np.max(np.abs(bond - 0.142)) < 1e-12                              # every bond has length a
+    # symmetric adjacency
+    pairs = set(zip(i[valid].tolist(), nl[valid].tolist()))
+    assert all((m, n) in pairs for n, m in pairs)
+
+
+def test_zgnr_config_counts():
+    cfg = W.make_config(6, shrink=64)
+    assert cfg.lattice.n == 1_048_576 // 64 and cfg.R == 1 and cfg.M == 2000
+    assert abs(cfg.period - 65536 // 64 * np.sqrt(3.0) * 0.142 / 2) < 1e-9      # L_x = sqrt(3) N_x a / 2 (P:91)

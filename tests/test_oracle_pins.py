@@ -602,3 +602,88 @@ def test_open_boundary_length_saturates_at_sample_length(kgo):
     assert np.max(open_[-4:]) > 0.6 * Lx
     assert np.min(pbc[-1]) > 1.5 * Lx
     assert np.all(np.diff(pbc.mean(axis=1)) > 0)
+
+
+# ------------------------------------------------------------------ zigzag ribbon (Fig. 4)
+def zgnr_bands(chains, nk=256):
+    """Bloch bands of a zigzag ribbon of `chains` zigzag chains from its textbook tight-binding strip
+    Hamiltonian (independent of any generator): 2*chains sites per unit cell; inside a chain the two
+    sublattice sites couple with t (1 + e^{-ik}), neighbouring chains couple with t through one bond."""
+    ks = np.linspace(-np.pi, np.pi, nk, endpoint=False)
+    n = 2 * chains
+    out = np.empty((nk, n))
+    for q, k in enumerate(ks):
+        h = np.zeros((n, n), complex)
+        for c in range(chains):
+            h[2 * c, 2 * c + 1] = T * (1 + np.exp(-1j * k))
+            if c + 1 < chains:
+                h[2 * c + 1, 2 * c + 2] = T
+        h = h + h.conj().T
+        out[q] = np.linalg.eigvalsh(h)
+    return ks, out
+
+
+def test_zgnr_flat_edge_band(kgo):
+    """ZGNR of 16 chains x 16 cells = 512 sites: the zero-energy edge band.  Textbook (Fujita et al.;
+    the flat band the paper's Fig. 4 b shows as the DOS peak at E = 0): edge states exist for
+    2 pi/3 < |k| <= pi, one per edge and k.  With 16 k-points that is 5 k-points x 2 edges = 10 states
+    within 0.1 eV of zero.  Checked (i) on the dense spectrum of the generated lattice, (ii) against the
+    strip Hamiltonian's bands, (iii) as the weight of the E = 0 peak in the oracle's KPM DOS."""
+    ncx, chains = 16, 16
+    lat = kgo.zgnr(ncx, chains)
+    assert lat.n == 512
+    _, E, _ = eig(lat)
+    k_edge = [j for j in range(-ncx // 2, ncx // 2) if abs(2 * np.pi * j / ncx) > 2 * np.pi / 3]
+    want = 2 * len(k_edge)
+    assert want == 10
+    assert np.sum(np.abs(E) < 0.1) == want
+    # the same levels from the strip Hamiltonian at the ribbon's allowed k
+    ks, bands = zgnr_bands(chains, nk=ncx)
+    assert np.max(np.abs(np.sort(bands.ravel()) - E)) < 1e-10
+    # oracle: full trace of T_n over unit vectors -> rho(E); weight of the peak at E = 0
+    M, s = 1200, S_GRAPHENE
+    mu = np.zeros(M)
+    for i in range(0, lat.n, 1):
+        if i % (2 * chains) >= 2 * chains:      # (all sites; translation symmetry is not assumed)
+            continue
+        phi = np.zeros(lat.n, complex); phi[i] = 1.0
+        mu += kgo.dos_moments(lat, 0.0, s, phi, M).real
+    mu /= lat.n
+    assert relerr(mu, np.array([np.mean(cheb_T(m, E / s)) for m in range(M)])) < 1e-11
+    en = np.linspace(-0.1, 0.1, 401)
+    rho = kgo.kpm_reconstruct(mu.astype(complex), 0.0, s, en)
+    weight = np.trapezoid(rho, en)
+    # Jackson width pi s / M = 0.022 eV: the ten levels (|E| <= 0.037 eV) sit well inside the window
+    assert abs(weight * lat.n - want) < 0.5
+
+
+def test_zgnr_first_plateau_conductance(kgo):
+    """Ballistic conductance of the pristine ZGNR on its first plateau (Fig. 4 a): one open
+    channel for 0 < |E| < E_1, so G -> 1 x 2e^2/h "within a short correlation time" (once the t^2 term of
+    DeltaX^2 dominates the bounded inter-band oscillations), from the oracle's Einstein chain kgo_msd ->
+    kgo_kpm_reconstruct -> kgo_transport.  The trace is exact: the ribbon is translation invariant along
+    x, so the average over the 32 sites of one unit cell of site-localised states IS Tr[...]/N."""
+    chains, ncx = 16, 320
+    lat = kgo.zgnr(ncx, chains)
+    _, bands = zgnr_bands(chains, nk=400)
+    # bottom of the second conduction subband: between the edge band and it there is a single band
+    pos = np.sort(bands, axis=1)[:, chains:]                  # conduction bands, ascending per k
+    e1 = pos[:, 1].min()
+    assert 0.5 < e1 < 1.2
+    en = np.array([0.5 * e1, 0.7 * e1])
+    en = np.concatenate([-en[::-1], en])
+    s, M, nt, dt = S_GRAPHENE, 500, 12, 8 * HBAR / 2.7
+    cell = [i for i in range(lat.n) if lat.x[i] < lat.x.min() + 0.2]       # the two x-columns of one unit cell
+    assert len(cell) == 2 * chains
+    rho = np.zeros(len(en)); fmsd = np.zeros((nt + 1, len(en)))
+    for i in cell:
+        phi = np.zeros(lat.n, complex); phi[i] = 1.0
+        rho += kgo.kpm_reconstruct(kgo.dos_moments(lat, 0.0, s, phi, M), 0.0, s, en)
+        mu = kgo.msd(lat, lat.x, lat.period_x, 0.0, s, phi, M, nt, dt)
+        fmsd += np.stack([kgo.kpm_reconstruct(mu[k], 0.0, s, en) for k in range(nt + 1)])
+    rho /= len(cell); fmsd /= len(cell)
+    out = kgo.transport(rho, None, fmsd, dt, 2.0 * lat.n / lat.period_x, 1.0)
+    g = out["conductance"] / 2.0                               # in 2e^2/h
+    assert 2 * np.sqrt(np.max(fmsd[-1] / rho)) < 0.45 * lat.period_x       # the wave packet has not wrapped around
+    print("ZGNR first plateau G/(2e^2/h) at t_k, k = 6, 9, 12:", np.round(g[[6, 9, 12]], 4))
+    assert np.max(np.abs(g[6:] - 1.0)) < 0.05
