@@ -1,5 +1,5 @@
 #!/usr/bin/env python
-"""Writes the stored oracle outputs (tests/golden/c*_*.npz) for BASELINE.json configs 2-5.
+"""Writes the stored oracle outputs (tests/golden/c*_*.npz) for BASELINE.json configs 2-5 and the paper's ZGNR (config 6 of workloads.make_config).
 
     python tests/golden/make_goldens.py --all --jobs 6         # every piece, 6 oracle processes
     python tests/golden/make_goldens.py --piece c4_msd_v0      # one piece in this process
@@ -23,6 +23,7 @@ config | lattice                                   | vectors | M    | N_t | M'
    3   | AGNR 15 x 20000 cells                     | 0       | 2000 | 400 | 64
    4   | 1000x1000 cells, Anderson W=|t| (seed 2)  | 0       | 3000 | 100 | 64
    5   | 2000x2000 cells, 0.1 % vacancies (seed 3) | 0, 7    | 3000 |  50 | 16
+   6   | ZGNR 65536 x 16 (the paper's Fig. 4)      | 0       | 2000 | 400 | 64
 
 Every file records the sha256 of oracle/kgo.c, the git commit of the tree that wrote it, the config
 parameters and the sha256 of the random vector's bytes.  Host time on 8 cores: about 1.5 h.
@@ -52,6 +53,7 @@ CONFIGS = {
     3: dict(vectors=(0,), M=2000, nt=400, dt_mult=1, Mp=64, seed=0, wants=("dos", "msd")),
     4: dict(vectors=(0,), M=3000, nt=100, dt_mult=4, Mp=64, seed=2, wants=("dos", "vac", "msd")),
     5: dict(vectors=(0, 7), M=3000, nt=50, dt_mult=8, Mp=16, seed=3, wants=("dos", "msd")),
+    6: dict(vectors=(0,), M=2000, nt=400, dt_mult=1, Mp=64, seed=0, wants=("dos", "msd")),
 }
 
 
@@ -77,6 +79,9 @@ def lattice(idx, shrink=1):
         nv = int(np.floor(0.001 * full.n + 0.5))
         lat = kgo.remove_sites(full, kgo.vacancy_mask(full.n, nv, 3))
         return lat, lat.x, lat.period_x, s
+    if idx == 6:
+        lat = kgo.zgnr(32768 // shrink, 16)
+        return lat, lat.x, lat.period_x, s
     raise ValueError(idx)
 
 
@@ -100,8 +105,8 @@ def cost(piece):
     """Rough oracle cost (H-type sweeps x sites) used to start the longest pieces first."""
     idx, job = int(piece[1]), piece.split("_")[1]
     c = CONFIGS[idx]
-    n = {2: 0.25e6, 3: 1.2e6, 4: 4e6, 5: 16e6}[idx]
-    n_p = {2: 28, 3: 21, 4: 42, 5: 57}[idx]
+    n = {2: 0.25e6, 3: 1.2e6, 4: 4e6, 5: 16e6, 6: 1.05e6}[idx]
+    n_p = {2: 28, 3: 21, 4: 42, 5: 57, 6: 21}[idx]
     if job == "dos":
         return n * c["M"]
     per_step = (5 if job == "msd" else 2) * n_p + c["Mp"]
