@@ -677,6 +677,46 @@ struct TmpDev {
     }
 };
 
+// Stream-ordered temporaries of the handle-free post-processing calls: cudaMallocAsync from the
+// device's default pool (kept warm: release threshold = never), cudaFreeAsync when the call
+// returns — no cudaMalloc, no cudaFree and no synchronisation once the pool has grown.
+struct AsyncTmp {
+    cudaStream_t st;
+    std::vector<void *> ptrs;
+    explicit AsyncTmp(cudaStream_t s) : st(s)
+    {
+        static bool pool_configured[64] = {false};
+        int dev = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < 64 && !pool_configured[dev]) {
+            cudaMemPool_t pool;
+            if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+                uint64_t keep = UINT64_MAX;
+                cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+            }
+            pool_configured[dev] = true;
+        }
+    }
+    ~AsyncTmp() { for (void *p : ptrs) cudaFreeAsync(p, st); }
+    int alloc(size_t bytes, void **d)
+    {
+        CUDA_TRY(cudaMallocAsync(d, bytes ? bytes : 16, st));
+        ptrs.push_back(*d);
+        return KG_OK;
+    }
+    // device view of an input: the pointer itself, or a stream-ordered copy of host memory
+    int get(const void *src, size_t bytes, const void **dev)
+    {
+        if (!src) { *dev = nullptr; return KG_OK; }
+        if (is_device_ptr(src)) { *dev = src; return KG_OK; }
+        void *d = nullptr;
+        int rc = alloc(bytes, &d);
+        if (rc) return rc;
+        CUDA_TRY(cudaMemcpyAsync(d, src, bytes, cudaMemcpyHostToDevice, st));
+        *dev = d;
+        return KG_OK;
+    }
+};
+
 extern "C" int kg_create_hamiltonian(kg_hamiltonian **out, int64_t n, int32_t kmax, const int32_t *nn,
                                      const int32_t *nl, const double *hop_eV, const double *onsite_eV,
                                      const double *x_nm, double period_x_nm, double e0_eV,
@@ -1301,29 +1341,27 @@ extern "C" int kg_kpm_reconstruct(const kg_c128 *mu, int64_t rows, int M, int ja
     if (!(scale_eV > 0.0) || !std::isfinite(scale_eV) || !std::isfinite(e0_eV))
         return fail(KG_EINVAL, "kg_kpm_reconstruct: scale must be positive and finite");
     cudaStream_t st = (cudaStream_t)stream;
-    std::vector<double> en((size_t)n_energies);
-    CUDA_TRY(cudaMemcpyAsync(en.data(), energies_eV, (size_t)n_energies * 8, cudaMemcpyDefault, st));
-    CUDA_TRY(cudaStreamSynchronize(st));
-    for (double e : en)
-        if (!(std::fabs((e - e0_eV) / scale_eV) < 1.0))
-            return fail(KG_EINVAL, "kg_kpm_reconstruct: energy %.6g eV is outside (E0 - s, E0 + s)", e);
-    TmpDev tmp;
+    // |x_j| < 1 is checked here when the grid is host memory; a device grid is not read back (no
+    // synchronisation): energies outside (E0 - s, E0 + s) then give NaN, from sqrt(1 - x^2)
+    if (!is_device_ptr(energies_eV))
+        for (int j = 0; j < n_energies; ++j)
+            if (!(std::fabs((energies_eV[j] - e0_eV) / scale_eV) < 1.0))
+                return fail(KG_EINVAL, "kg_kpm_reconstruct: energy %.6g eV is outside (E0 - s, E0 + s)", energies_eV[j]);
+    AsyncTmp tmp(st);
     const void *d_mu, *d_en;
     int rc;
-    if ((rc = tmp.get(mu, (size_t)rows * M * 16, st, &d_mu)) || (rc = tmp.get(energies_eV, (size_t)n_energies * 8, st, &d_en)))
+    if ((rc = tmp.get(mu, (size_t)rows * M * 16, &d_mu)) || (rc = tmp.get(energies_eV, (size_t)n_energies * 8, &d_en)))
         return rc;
-    double *d_w = nullptr, *d_f = nullptr;
-    CUDA_TRY(cudaMalloc(&d_w, (size_t)M * 8)); tmp.ptrs.push_back(d_w);
+    void *d_w = nullptr, *d_f = f;
+    if ((rc = tmp.alloc((size_t)M * 8, &d_w))) return rc;
     const bool f_dev = is_device_ptr(f);
-    if (f_dev) d_f = f;
-    else { CUDA_TRY(cudaMalloc(&d_f, (size_t)rows * n_energies * 8)); tmp.ptrs.push_back(d_f); }
-    kg_kpm_weights<<<(M + 255) / 256, 256, 0, st>>>(M, jackson, d_w);
+    if (!f_dev && (rc = tmp.alloc((size_t)rows * n_energies * 8, &d_f))) return rc;
+    kg_kpm_weights<<<(M + 255) / 256, 256, 0, st>>>(M, jackson, (double *)d_w);
     dim3 grid((n_energies + 127) / 128, (unsigned)rows);
-    kg_kpm_reconstruct_kernel<<<grid, 128, 0, st>>>((const c128 *)d_mu, rows, M, d_w, e0_eV, scale_eV,
-                                                    (const double *)d_en, n_energies, d_f);
+    kg_kpm_reconstruct_kernel<<<grid, 128, 0, st>>>((const c128 *)d_mu, rows, M, (const double *)d_w, e0_eV, scale_eV,
+                                                    (const double *)d_en, n_energies, (double *)d_f);
     CUDA_TRY(cudaGetLastError());
     if (!f_dev) CUDA_TRY(cudaMemcpyAsync(f, d_f, (size_t)rows * n_energies * 8, cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(cudaStreamSynchronize(st));     // temporaries are freed on return
     return KG_OK;
 }
 
@@ -1341,19 +1379,20 @@ extern "C" int kg_transport(int n_steps, int n_energies, double dt_fs, double de
     if ((length_nm || conductance) && !rho) return fail(KG_EINVAL, "kg_transport: length / conductance need rho");
     cudaStream_t st = (cudaStream_t)stream;
     const size_t tbytes = (size_t)(n_steps + 1) * n_energies * 8;
-    TmpDev tmp;
+    AsyncTmp tmp(st);
     const void *d_rho, *d_vac, *d_msd;
     int rc;
-    if ((rc = tmp.get(rho, (size_t)n_energies * 8, st, &d_rho)) || (rc = tmp.get(sigma_gk ? fvac : nullptr, tbytes, st, &d_vac)) ||
-        (rc = tmp.get(fmsd, tbytes, st, &d_msd)))
+    if ((rc = tmp.get(rho, (size_t)n_energies * 8, &d_rho)) || (rc = tmp.get(sigma_gk ? fvac : nullptr, tbytes, &d_vac)) ||
+        (rc = tmp.get(fmsd, tbytes, &d_msd)))
         return rc;
     double *user[5] = {sigma_gk, sigma_e1, sigma_e2, length_nm, conductance};
     double *dev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     for (int q = 0; q < 5; ++q) {
         if (!user[q]) continue;
         if (is_device_ptr(user[q])) { dev[q] = user[q]; continue; }
-        CUDA_TRY(cudaMalloc(&dev[q], tbytes));
-        tmp.ptrs.push_back(dev[q]);
+        void *d;
+        if ((rc = tmp.alloc(tbytes, &d))) return rc;
+        dev[q] = (double *)d;
     }
     kg_transport_kernel<<<(n_energies + 127) / 128, 128, 0, st>>>(n_steps, n_energies, dt_fs,
         2.0 * 3.14159265358979323846 * KG_HBAR * dens_per_nm2, width_nm, (const double *)d_rho,
@@ -1361,7 +1400,6 @@ extern "C" int kg_transport(int n_steps, int n_energies, double dt_fs, double de
     CUDA_TRY(cudaGetLastError());
     for (int q = 0; q < 5; ++q)
         if (user[q] && dev[q] != user[q]) CUDA_TRY(cudaMemcpyAsync(user[q], dev[q], tbytes, cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(cudaStreamSynchronize(st));
     return KG_OK;
 }
 
@@ -1433,21 +1471,19 @@ extern "C" int kg_ftm_reconstruct(const kg_c128 *F, int64_t rows, int Nm, int wi
         return fail(KG_EINVAL, "kg_ftm_reconstruct: need 1 <= rows <= 65535, Nm >= 0, n_energies >= 1");
     if (!(dtau_fs > 0.0) || !std::isfinite(dtau_fs)) return fail(KG_EINVAL, "dtau_fs must be finite and positive");
     cudaStream_t st = (cudaStream_t)stream;
-    TmpDev tmp;
+    AsyncTmp tmp(st);
     const void *d_F, *d_en;
     int rc;
-    if ((rc = tmp.get(F, (size_t)rows * (2 * Nm + 1) * 16, st, &d_F)) ||
-        (rc = tmp.get(energies_eV, (size_t)n_energies * 8, st, &d_en)))
+    if ((rc = tmp.get(F, (size_t)rows * (2 * Nm + 1) * 16, &d_F)) ||
+        (rc = tmp.get(energies_eV, (size_t)n_energies * 8, &d_en)))
         return rc;
-    double *d_f = nullptr;
+    void *d_f = f;
     const bool f_dev = is_device_ptr(f);
-    if (f_dev) d_f = f;
-    else { CUDA_TRY(cudaMalloc(&d_f, (size_t)rows * n_energies * 8)); tmp.ptrs.push_back(d_f); }
+    if (!f_dev && (rc = tmp.alloc((size_t)rows * n_energies * 8, &d_f))) return rc;
     dim3 grid((n_energies + 127) / 128, (unsigned)rows);
     kg_ftm_reconstruct_kernel<<<grid, 128, 0, st>>>((const c128 *)d_F, rows, Nm, window, dtau_fs / KG_HBAR,
-                                                    (const double *)d_en, n_energies, d_f);
+                                                    (const double *)d_en, n_energies, (double *)d_f);
     CUDA_TRY(cudaGetLastError());
     if (!f_dev) CUDA_TRY(cudaMemcpyAsync(f, d_f, (size_t)rows * n_energies * 8, cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(cudaStreamSynchronize(st));
     return KG_OK;
 }

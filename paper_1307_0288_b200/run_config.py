@@ -25,14 +25,15 @@ import numpy as np
 
 # which correlation functions each config asks for (BASELINE.json "configs")
 WANTS = {1: ("dos", "vac", "msd"), 2: ("dos", "vac", "msd"), 3: ("dos", "msd"),
-         4: ("dos", "vac", "msd"), 5: ("dos", "msd")}
+         4: ("dos", "vac", "msd"), 5: ("dos", "msd"), 6: ("dos", "msd")}
 A_NM = 0.142
 GRAPHENE_DENS = 8.0 / (3.0 * np.sqrt(3.0) * A_NM ** 2)      # 2N/Omega of a honeycomb sheet, nm^-2
 
 
 def main(argv=None):
     ap = argparse.ArgumentParser(description=__doc__.split("\n\n")[0])
-    ap.add_argument("--config", type=int, required=True, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--config", type=int, required=True, choices=[1, 2, 3, 4, 5, 6],
+                    help="BASELINE.json config 1..5, or 6 = the paper's ZGNR 65536 x 16 (Fig. 4)")
     ap.add_argument("--time-steps", type=int, default=None, help="override the config's number of time steps")
     ap.add_argument("--moments", type=int, default=None, help="override the config's M")
     ap.add_argument("--out", default=None, help="directory for <config name>.npz")
@@ -87,7 +88,7 @@ def main(argv=None):
         if "mu_msd" in res:
             fmsd = B.kpm_reconstruct(res["mu_msd"], cfg.e0, cfg.scale, energies).mean(dim=0).contiguous()
         if nt >= 1 and (fvac is not None or fmsd is not None):
-            if args.config == 3:
+            if args.config in (3, 6):
                 # ribbon of N sites and length L_s: dens * W = 2N/L_s, so with width_nm = 1 the
                 # conductance (W/L) sigma_E1 needs dens = 2N/(L_s * 1 nm)
                 dens, width = 2.0 * n / cfg.period, 1.0
@@ -120,7 +121,7 @@ def main(argv=None):
         summary["sigma_e2_over_e1_last"] = float(np.mean(host["sigma_e2"][nt - 1][inner]) /
                                                  np.mean(host["sigma_e1"][nt - 1][inner]))
         summary["length_nm_last_mean"] = float(np.mean(host["length_nm"][nt][inner]))
-    if args.config == 3 and "conductance" in host and nt >= 2:
+    if args.config in (3, 6) and "conductance" in host and nt >= 2:
         g = host["conductance"][nt - 1] / 2.0        # in 2e^2/h
         summary["G_2e2h_at_|E|<0.5eV_mean"] = float(np.mean(g[np.abs(en) < 0.5]))
         summary["G_2e2h_at_1.0-1.2eV_mean"] = float(np.mean(g[(np.abs(en) > 1.0) & (np.abs(en) < 1.2)]))

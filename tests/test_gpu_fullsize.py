@@ -267,3 +267,78 @@ def test_fig4_quantised_conductance_of_the_ribbon(B):
         assert np.all(ratio > 0.90) and np.all(ratio < 1.12), (k, ratio)     # measured 0.93-1.08 (4 vectors)
     e2_over_e1 = host(tr["sigma_e2"])[23][want > 0] / host(tr["sigma_e1"])[23][want > 0]
     assert np.all(np.abs(e2_over_e1 - 0.5) < 0.03)            # sigma_E2 = sigma_E1 / 2 when ballistic
+
+
+def zgnr_strip_bands(chains, nk):
+    """Bloch bands of a zigzag ribbon from its textbook strip Hamiltonian (2 * chains sites per unit
+    cell; t (1 + e^{-ik}) inside a chain, t between neighbouring chains)."""
+    t = -2.7
+    ks = np.linspace(-np.pi, np.pi, nk, endpoint=False)
+    out = np.empty((nk, 2 * chains))
+    for q, k in enumerate(ks):
+        h = np.zeros((2 * chains, 2 * chains), complex)
+        for c in range(chains):
+            h[2 * c, 2 * c + 1] = t * (1 + np.exp(-1j * k))
+            if c + 1 < chains:
+                h[2 * c + 1, 2 * c + 2] = t
+        out[q] = np.linalg.eigvalsh(h + h.conj().T)
+    return out
+
+
+def test_zgnr_prefix_parity(B, kgo):
+    """The paper's ZGNR at full size (65536 x 16 = 1 048 576 sites): DOS prefix and MSD rows 0..2
+    against the live oracle (the stored all-time-steps comparison is in test_gpu_goldens.py)."""
+    cfg = W.make_config(6)
+    lat = cfg.lattice
+    assert lat.n == 1_048_576
+    olat = to_oracle_lattice(kgo, lat)
+    h = B.from_lattice(lat, cfg.xcoord, cfg.period, cfg.e0, cfg.scale)
+    phi = W.random_phase_vectors(lat.n, 1, cfg.seed)
+    Mp, ntp = 24, 2
+    dos = host(B.dos_moments(h, dev(phi), Mp))[0]
+    msd = host(B.msd(h, dev(phi), Mp, ntp, cfg.dt_fs))[0]
+    v = phi[:, 0].copy()
+    assert relerr(dos, kgo.dos_moments(olat, 0.0, cfg.scale, v, Mp)) <= TOL
+    assert relerr(msd, kgo.msd(olat, cfg.xcoord, cfg.period, 0.0, cfg.scale, v, Mp, ntp, cfg.dt_fs)) <= TOL
+
+
+def test_fig4_zgnr_plateaus_and_edge_peak(B):
+    """Fig. 4 on the paper's own system, the pristine ZGNR 65536 x 16: (a) the Einstein
+    conductance G = (W/L) sigma_E1 (eqs 50-51) shows the odd plateaus 1, 3, 5 x 2e^2/h of a zigzag ribbon
+    at the plateau centres (channel count from the ribbon's textbook strip-Hamiltonian bands), with the
+    slight overestimate towards the subband edges the paper describes; (b) the flat edge band gives the DOS
+    peak at E = 0; sigma_E2 = sigma_E1 / 2 in the ballistic regime."""
+    import torch
+    cfg = W.make_config(6)
+    lat = cfg.lattice
+    h = B.from_lattice(lat, cfg.xcoord, cfg.period, 0.0, cfg.scale)
+    bands = zgnr_strip_bands(16, 1200)
+
+    def channels(E):
+        # right-movers at energy E: half of the band crossings on the closed k loop
+        sgn = np.sign(bands - E)
+        return int(np.sum(sgn != np.roll(sgn, 1, axis=0))) // 2
+
+    cond = np.sort(bands, axis=1)[:, 16:]                        # conduction bands per k, ascending
+    edges = np.sort(cond[:, 1:6].min(axis=0))                    # bottoms of subbands 2..6
+    # the p-th conduction subband (p >= 2) opens a channel pair: 1 | 3 | 5 ... between consecutive bottoms
+    mids = np.array([0.5 * edges[0], 0.5 * (edges[0] + edges[1]), 0.5 * (edges[1] + edges[2])])
+    assert [channels(x) for x in mids] == [1, 3, 5]
+    e = np.concatenate([-mids[::-1], [0.0], mids])
+    R, M, nt, dt = 4, 2000, 24, 4 * cfg.dt_fs
+    phi = dev(W.random_phase_vectors(lat.n, R, 5))
+    en = torch.from_numpy(e).cuda()
+    rho = B.kpm_reconstruct(B.dos_moments(h, phi, M), 0.0, cfg.scale, en).mean(dim=0).contiguous()
+    fmsd = B.kpm_reconstruct(B.msd(h, phi, M, nt, dt), 0.0, cfg.scale, en).mean(dim=0).contiguous()
+    tr = B.transport(rho, None, fmsd, dt, 2.0 * lat.n / cfg.period, 1.0)
+    g = host(tr["conductance"]) / 2.0                            # in units of 2e^2/h
+    want = np.array([channels(x) for x in e], float)
+    nz = want > 0
+    nz[3] = False                                                # E = 0: the flat band carries no current
+    for k in (8, 16, 23):
+        ratio = g[k][nz] / want[nz]
+        assert np.all(ratio > 0.90) and np.all(ratio < 1.15), (k, ratio)
+    e2_over_e1 = host(tr["sigma_e2"])[23][nz] / host(tr["sigma_e1"])[23][nz]
+    assert np.all(np.abs(e2_over_e1 - 0.5) < 0.03)
+    r = host(rho)
+    assert r[3] > 5 * r[[2, 4]].max()                            # Fig. 4 b: the edge-state peak at E = 0

@@ -60,14 +60,15 @@ def rowwise_err(got, want):
     return worst
 
 
-VECTORS = {2: (0, 3), 3: (0,), 4: (0,), 5: (0, 7)}
-WANTS = {2: ("vac", "msd"), 3: ("msd",), 4: ("vac", "msd"), 5: ("msd",)}
+VECTORS = {2: (0, 3), 3: (0,), 4: (0,), 5: (0, 7), 6: (0,)}
+WANTS = {2: ("vac", "msd"), 3: ("msd",), 4: ("vac", "msd"), 5: ("msd",), 6: ("msd",)}
 
 
-@pytest.mark.parametrize("idx", [2, 3, 4, 5])
+@pytest.mark.parametrize("idx", [2, 3, 4, 5, 6])
 def test_full_job_against_stored_oracle_outputs(B, idx):
     """The whole config — kg_dos_moments(M), kg_vac / kg_msd over ALL N_t time steps with ALL M
-    moments, all R vectors in one batch — compared on every stored oracle entry."""
+    moments, all R vectors in one batch — compared on every stored oracle entry.  idx 6 is the paper's
+    own ballistic system, the zigzag ribbon 65536 x 16 of Fig. 4 (workloads.make_config(6))."""
     import torch
     cfg = W.make_config(idx)
     lat = cfg.lattice
