@@ -18,24 +18,37 @@
  * cudaPointerGetAttributes.  Host inputs are copied to library-owned device staging
  * buffers on `stream`; host outputs are written by an asynchronous device->host copy on
  * `stream` (for pageable memory CUDA makes that copy synchronous).  All arithmetic runs in
- * CUDA kernels; there is no CPU fallback.  All arrays are caller-owned and only borrowed for
- * the duration of the call; inputs are never modified; `out` must not alias `in`.
+ * CUDA kernels; there is no CPU fallback.  All arrays are caller-owned and BORROWED IN STREAM
+ * ORDER: device arrays and pinned host arrays are read / written by work that is still queued
+ * on `stream` when the call returns, so they must stay alive and unmodified (inputs) / unread
+ * (outputs) until that work has run — synchronise the stream, or order later work after it on
+ * the same stream.  Pageable host arrays are consumed / filled before the call returns.
+ * Inputs are never modified; `out` must not alias `in`.
  *
  * VECTORS are `[n][R]` complex128, site-major (the R values of one site are contiguous,
- * element (site i, vector r) at index i*R + r), R in {1, 2, 4, 8} (kg_evolve and
- * kg_apply_velocity also accept 16).  kg_c128 is layout-compatible with C99 `double complex`,
- * std::complex<double> and torch.complex128.
+ * element (site i, vector r) at index i*R + r), R in {1, 2, 4, 8, 16}; kg_vac takes R <= 8
+ * (it advances [psi | chi] as one batch of 2R columns).  kg_c128 is layout-compatible with
+ * C99 `double complex`, std::complex<double> and torch.complex128.  The sites may be
+ * re-numbered inside the library (KG_OPT_REORDER); every vector crosses this boundary in the
+ * CALLER's site order.
  *
  * STREAMS.  `stream` is a cudaStream_t cast to void* (NULL = legacy default stream).  Calls
- * enqueue work on it and return without synchronising, except kg_create_hamiltonian (which
- * validates and therefore synchronises) and calls whose outputs are pageable host memory.
- * Device outputs are valid once the stream has been synchronised.
+ * enqueue work on it and return without synchronising, except: kg_create_hamiltonian[_csr]
+ * (validation result), the first moments call of a handle that builds the two-step kernel's
+ * tile plan (KG_OPT_TWO_STEP), calls that have to grow the workspace while a cached CUDA graph
+ * refers to it, calls with KG_OPT_CHECK_INPUT set, and calls whose outputs are pageable host
+ * memory.  Device outputs are valid once the stream has been synchronised.
  *
  * ERRORS.  Every call returns KG_OK or an error code; nothing throws or aborts across the
- * ABI.  kg_last_error() returns a thread-local description of the last failure.
+ * ABI (the bodies run inside a catch-all guard: a failed host allocation is KG_ENOMEM).
+ * kg_last_error() returns a thread-local description of the last failure.
  *
  * A handle owns its device copy of the matrix and a lazily grown workspace (Chebyshev
- * vectors T_m, accumulators, per-block moment partials).  A handle is not thread-safe.
+ * vectors T_m, accumulators, per-block moment partials, cached CUDA graphs) that every call
+ * on the handle re-uses: a handle is not thread-safe, and its calls must be issued on ONE
+ * stream at a time (before switching streams, synchronise the old one or make the new one
+ * wait on an event recorded in it) — two calls on different streams would race on the
+ * workspace.  Different handles are independent.
  */
 #ifndef KG_H
 #define KG_H
@@ -111,8 +124,9 @@ int64_t kg_num_sites(const kg_hamiltonian *h);
  * (Alg. 5, eq 46).  <a|b> = sum_i conj(a_i) b_i.
  *   phiL, phiR  [n][R]; may be the same pointer
  *   mu          [R][M] complex128 (vector r at mu[r*M + m]), M >= 2
- * One fused kernel per Chebyshev step (recursion eq 38 + inner product) and a final
- * fixed-order reduction: results are bitwise reproducible run to run.
+ * One fused kernel per Chebyshev step (recursion eq 38 + inner product) — or per two steps,
+ * KG_OPT_TWO_STEP — and a final fixed-order reduction: results are bitwise reproducible run to
+ * run for a given handle and option set.
  */
 int kg_moments(kg_hamiltonian *h, const kg_c128 *phiL, const kg_c128 *phiR, int R, int M,
                kg_c128 *mu, void *stream);
@@ -181,9 +195,11 @@ int kg_bessel_terms(double x, double bessel_eps, int *np_out, double *j, int cap
  * of kg_vac / kg_msd it gives rho(E) C_vv(E,t) (nm^2/fs^2/eV) / rho(E) DeltaX^2(E,t) (nm^2/eV).
  *   mu        [rows][M] complex128 (any leading shape flattened to rows), host or device
  *   jackson   1: g_m as above; 0: g_m = 1 (Dirichlet)
- *   energies_eV [n_energies], host or device; every |x_j| must be < 1 (else KG_EINVAL)
+ *   energies_eV [n_energies], host or device; every |x_j| must be < 1: a host grid is checked
+ *             (KG_EINVAL), a device grid is not read back — such entries of f are NaN
  *   f         [rows][n_energies] fp64, host or device
- * Runs as CUDA kernels on `stream` and synchronises it before returning.
+ * Runs as CUDA kernels on `stream`; temporaries are stream-ordered pool allocations
+ * (cudaMallocAsync), so the call neither allocates with cudaMalloc nor synchronises.
  */
 int kg_kpm_reconstruct(const kg_c128 *mu, int64_t rows, int M, int jackson, double e0_eV,
                        double scale_eV, const double *energies_eV, int n_energies, double *f,
@@ -202,7 +218,9 @@ int kg_kpm_reconstruct(const kg_c128 *mu, int64_t rows, int M, int jackson, doub
  *   length_nm = 2 sqrt(fmsd / rho)                           (eq 50)
  *   conductance = (width_nm / length_nm) * sigma_e1, 0 where the length is 0  (eq 51)
  * All arrays fp64, host or device; tables are [n_steps+1][n_energies].  Every output pointer may
- * be NULL; fvac (fmsd, rho) may be NULL when no requested output needs it.  Synchronises `stream`.
+ * be NULL; fvac (fmsd, rho) may be NULL when no requested output needs it.  Does not synchronise.
+ * The stochastic trace average over random vectors (eq 21) is the caller's: average the
+ * reconstructed rows over vectors before this call (the functions are linear in the moments).
  */
 int kg_transport(int n_steps, int n_energies, double dt_fs, double dens_per_nm2, double width_nm,
                  const double *rho, const double *fvac, const double *fmsd, double *sigma_gk,
@@ -226,14 +244,16 @@ int kg_fourier_moments(kg_hamiltonian *h, const kg_c128 *phiL, const kg_c128 *ph
  * and spin for unit-norm phi:
  *   f[row][j] = dtau/(2 pi hbar) * sum_{n=-Nm}^{Nm} w_n Re[ exp(i E_j n dtau/hbar) F[row][n+Nm] ].
  *   F [rows][2*Nm+1], energies_eV [n_energies], f [rows][n_energies]; host or device pointers.
- * Synchronises `stream` before returning.
+ * Does not synchronise.
  */
 int kg_ftm_reconstruct(const kg_c128 *F, int64_t rows, int Nm, int window, double dtau_fs,
                        const double *energies_eV, int n_energies, double *f, void *stream);
 
 /* Tuning / introspection (not part of the paper's problem statement). */
 enum {
-    KG_OPT_USE_GRAPHS = 1,   /* 1 (default): replay the moment loop as a CUDA graph */
+    KG_OPT_USE_GRAPHS = 1,   /* replay the one-step moment loop as a cached CUDA graph: 1 always, 0 never, -1 (default)
+                                when n * R <= 2^21 (launch-bound sizes); never on the legacy default stream, which
+                                cannot be captured */
     KG_OPT_BLOCKS_PER_SM = 2, /* persistent grid = SMs * this (default chosen per kernel) */
     KG_OPT_THREADS = 3,      /* threads per block (default 256) */
     KG_OPT_STAGED = 4,       /* 1 (default): moment steps run the TMA-staged kernel when eligible */
@@ -257,6 +277,9 @@ enum {
                                 pass with the tile + two halo rings in shared memory (temporal blocking):
                                 1 whenever the plan fits, 0 never, -1 (default) when the sites are re-ordered
                                 and there are at least four 1024-element tiles per SM */
+    KG_OPT_CHECK_INPUT = 14, /* 1: every input vector is scanned for NaN / Inf (one extra pass and a stream
+                                synchronisation per call) and the call returns KG_EINVAL; 0 (default): not checked —
+                                non-finite input gives non-finite output.  (The matrix is always checked at create.) */
     KG_OPT_PDL = 11          /* consecutive sweeps chained by programmatic dependent launch (the next sweep's
                                 CTAs are scheduled while this one drains): 1 on, 0 off, -1 (default) on for
                                 launch-bound sizes, n * R <= 2^18 */

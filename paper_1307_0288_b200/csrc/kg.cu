@@ -30,6 +30,22 @@ static int fail(int code, const char *fmt, ...)
     return code;
 }
 
+// Nothing may throw across the C ABI: the bodies of the extern "C" calls run inside this guard
+// (std::vector growth in the host-side tables can throw std::bad_alloc).
+template <class F>
+static int guarded(F &&body)
+{
+    try {
+        return body();
+    } catch (const std::bad_alloc &) {
+        return fail(KG_ENOMEM, "host allocation failed");
+    } catch (const std::exception &e) {
+        return fail(KG_ECUDA, "internal error: %s", e.what());
+    } catch (...) {
+        return fail(KG_ECUDA, "internal error");
+    }
+}
+
 #define CUDA_TRY(expr)                                                                        \
     do {                                                                                      \
         cudaError_t e_ = (expr);                                                              \
@@ -47,10 +63,12 @@ static int g_reorder = -1;                    // KG_OPT_REORDER: -1 auto, 0 off,
 
 extern "C" int kg_set_default_option(int option, int64_t value)
 {
+    return guarded([&]() -> int {
     switch (option) {
     case KG_OPT_REORDER: g_reorder = value < 0 ? -1 : (value != 0); return KG_OK;
     }
     return fail(KG_EINVAL, "kg_set_default_option: option %d has no process-wide default", option);
+    });
 }
 
 // --------------------------------------------------------------------------------------
@@ -98,6 +116,8 @@ struct kg_hamiltonian {
     int ndict;                // entries in use (0: hoppings do not fit a dictionary)
     int staged, stages, staged_ctas, alternate, doubling, clenshaw, pdl;   // options of the staged kernel
     int tb2;                  // KG_OPT_TWO_STEP: -1 auto, 0 off, 1 whenever a plan exists
+    int check_input;          // KG_OPT_CHECK_INPUT: input vectors are scanned for NaN / Inf (one pass + a synchronisation)
+    unsigned int *d_flag;     // device flag of that scan
     Tb2Plan tbp[2];
     void *ws[WS_COUNT];
     size_t ws_bytes[WS_COUNT];
@@ -142,7 +162,23 @@ static int grid_for(const kg_hamiltonian *h, int64_t elems);
 // Internal-order device view of a caller vector [n][R] (host or device pointer, caller's site order):
 // the pointer itself when it is a device pointer and the sites are not re-ordered; else a copy in
 // workspace slot `slot` (host -> device copy and / or the permutation kernel).
+static int vec_in_raw(kg_hamiltonian *h, int slot, const void *p, int R, cudaStream_t st, const void **dev);
 static int vec_in(kg_hamiltonian *h, int slot, const void *p, int R, cudaStream_t st, const void **dev)
+{
+    int rc = vec_in_raw(h, slot, p, R, st, dev);
+    if (rc || !h->check_input) return rc;
+    // KG_OPT_CHECK_INPUT: "non-finite input -> KG_EINVAL" for state vectors costs one pass and a synchronisation
+    if (!h->d_flag) CUDA_TRY(cudaMalloc(&h->d_flag, 4));
+    CUDA_TRY(cudaMemsetAsync(h->d_flag, 0, 4, st));
+    kg_check_finite<<<grid_for(h, h->n * R), 256, 0, st>>>((const double *)*dev, h->n * R * 2, h->d_flag);
+    h->launches++;
+    unsigned int bad = 0;
+    CUDA_TRY(cudaMemcpyAsync(&bad, h->d_flag, 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (bad) return fail(KG_EINVAL, "input vector holds a non-finite value");
+    return KG_OK;
+}
+static int vec_in_raw(kg_hamiltonian *h, int slot, const void *p, int R, cudaStream_t st, const void **dev)
 {
     const size_t bytes = (size_t)h->n * R * 16;
     const bool on_dev = is_device_ptr(p);
@@ -495,12 +531,14 @@ static void bessel_table(double x, double eps, std::vector<double> &j)
 
 extern "C" int kg_bessel_terms(double x, double bessel_eps, int *np_out, double *j, int cap)
 {
+    return guarded([&]() -> int {
     if (!np_out || !std::isfinite(x)) return fail(KG_EINVAL, "kg_bessel_terms: bad argument");
     std::vector<double> t;
     bessel_table(x, bessel_eps, t);
     *np_out = (int)t.size();
     if (j) for (int m = 0; m < (int)t.size() && m < cap; ++m) j[m] = t[m];
     return KG_OK;
+    });
 }
 
 // c_m = (2 - delta_m0) (-+ i)^m J_m(x) * exp(-i E0 dt/hbar), upper sign for dt > 0 (eq 36)
@@ -542,6 +580,7 @@ static int create_from_device_list(kg_hamiltonian **out, int64_t n, int kmax, co
     h->nl = h->nlp = nullptr; h->hop = h->xhop = h->onsite = nullptr;
     h->perm = h->iperm = nullptr;
     h->tb2 = -1; memset(h->tbp, 0, sizeof(h->tbp));
+    h->check_input = 0; h->d_flag = nullptr;
     h->ndict = 0; h->staged = 1; h->stages = 0; h->staged_ctas = 0; h->alternate = 1; h->doubling = 1; h->clenshaw = 1; h->pdl = -1;
     memset(h->dict, 0, sizeof(h->dict));
     memset(h->ws, 0, sizeof(h->ws));
@@ -722,6 +761,7 @@ extern "C" int kg_create_hamiltonian(kg_hamiltonian **out, int64_t n, int32_t km
                                      const double *x_nm, double period_x_nm, double e0_eV,
                                      double scale_eV, void *stream)
 {
+    return guarded([&]() -> int {
     int rc = check_create_args(out, n, kmax, nn, nl, hop_eV, x_nm, period_x_nm, e0_eV, scale_eV);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
@@ -734,6 +774,7 @@ extern "C" int kg_create_hamiltonian(kg_hamiltonian **out, int64_t n, int32_t km
     return create_from_device_list(out, n, kmax, (const int32_t *)d_nn, (const int32_t *)d_nl,
                                    (const double *)d_hop, (const double *)d_ons, (const double *)d_x,
                                    period_x_nm, e0_eV, scale_eV, st);
+    });
 }
 
 extern "C" int kg_create_hamiltonian_csr(kg_hamiltonian **out, int64_t n, const int64_t *rowptr,
@@ -741,6 +782,7 @@ extern "C" int kg_create_hamiltonian_csr(kg_hamiltonian **out, int64_t n, const 
                                          const double *onsite_eV, const double *x_nm,
                                          double period_x_nm, double e0_eV, double scale_eV, void *stream)
 {
+    return guarded([&]() -> int {
     int rc = check_create_args(out, n, 1, rowptr, col, hop_eV, x_nm, period_x_nm, e0_eV, scale_eV);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
@@ -776,6 +818,7 @@ extern "C" int kg_create_hamiltonian_csr(kg_hamiltonian **out, int64_t n, const 
     CUDA_TRY(cudaGetLastError());
     return create_from_device_list(out, n, kmax, d_nn, d_nl, d_hop, (const double *)d_ons,
                                    (const double *)d_x, period_x_nm, e0_eV, scale_eV, st);
+    });
 }
 
 extern "C" int kg_destroy_hamiltonian(kg_hamiltonian *h)
@@ -783,7 +826,7 @@ extern "C" int kg_destroy_hamiltonian(kg_hamiltonian *h)
     if (!h) return KG_OK;
     for (auto &g : h->graphs) cudaGraphExecDestroy(g.exec);
     cudaFree(h->nl); cudaFree(h->nlp); cudaFree(h->hop); cudaFree(h->xhop); cudaFree(h->onsite);
-    cudaFree(h->perm); cudaFree(h->iperm);
+    cudaFree(h->perm); cudaFree(h->iperm); cudaFree(h->d_flag);
     for (auto &tp : h->tbp) { cudaFree(tp.tinfo); cudaFree(tp.rows); cudaFree(tp.hid); cudaFree(tp.hons); }
     for (int i = 0; i < WS_COUNT; ++i) cudaFree(h->ws[i]);
     delete h;
@@ -803,6 +846,7 @@ extern "C" int64_t kg_launch_count(const kg_hamiltonian *h) { return h ? h->laun
 
 extern "C" int kg_set_option(kg_hamiltonian *h, int option, int64_t value)
 {
+    return guarded([&]() -> int {
     if (!h) return fail(KG_EINVAL, "NULL handle");
     switch (option) {
     case KG_OPT_USE_GRAPHS: h->use_graphs = (int)value; break;
@@ -824,6 +868,7 @@ extern "C" int kg_set_option(kg_hamiltonian *h, int option, int64_t value)
     case KG_OPT_CLENSHAW: h->clenshaw = value != 0; break;
     case KG_OPT_PDL: h->pdl = value < 0 ? -1 : (value != 0); break;
     case KG_OPT_TWO_STEP: h->tb2 = value < 0 ? -1 : (value != 0); break;
+    case KG_OPT_CHECK_INPUT: h->check_input = value != 0; break;
     case KG_OPT_DICT:
         if (value != 0) return fail(KG_EINVAL, "the dictionary can only be switched off");
         h->ndict = 0; break;
@@ -832,6 +877,7 @@ extern "C" int kg_set_option(kg_hamiltonian *h, int option, int64_t value)
     for (auto &g : h->graphs) cudaGraphExecDestroy(g.exec);
     h->graphs.clear();
     return KG_OK;
+    });
 }
 
 // --------------------------------------------------------------------------------------
@@ -1162,8 +1208,9 @@ static int finish_out(const OutStage &o, cudaStream_t st)
 extern "C" int kg_moments(kg_hamiltonian *h, const kg_c128 *phiL, const kg_c128 *phiR, int R, int M,
                           kg_c128 *mu, void *stream)
 {
+    return guarded([&]() -> int {
     if (!h || !phiL || !phiR || !mu) return fail(KG_EINVAL, "kg_moments: NULL argument");
-    if (!r_ok(R, false)) return fail(KG_EUNSUPPORTED, "R must be 1, 2, 4 or 8");
+    if (!r_ok(R, true)) return fail(KG_EUNSUPPORTED, "R must be 1, 2, 4, 8 or 16");
     if (M < 2) return fail(KG_EINVAL, "M must be >= 2");
     cudaStream_t st = (cudaStream_t)stream;
     const void *dL, *dR;
@@ -1175,16 +1222,20 @@ extern "C" int kg_moments(kg_hamiltonian *h, const kg_c128 *phiL, const kg_c128 
     if ((rc = stage_out(h, WS_MU, mu, (size_t)R * M * 16, &o))) return rc;
     if ((rc = moments_device(h, (const c128 *)dL, R, (const c128 *)dR, R, R, M, (c128 *)o.dev, M, st))) return rc;
     return finish_out(o, st);
+    });
 }
 
 extern "C" int kg_dos_moments(kg_hamiltonian *h, const kg_c128 *phi, int R, int M, kg_c128 *mu, void *stream)
 {
+    return guarded([&]() -> int {
     return kg_moments(h, phi, phi, R, M, mu, stream);
+    });
 }
 
 extern "C" int kg_evolve(kg_hamiltonian *h, const kg_c128 *in, kg_c128 *out, int R, double dt_fs,
                          double bessel_eps, void *stream)
 {
+    return guarded([&]() -> int {
     if (!h || !in || !out) return fail(KG_EINVAL, "kg_evolve: NULL argument");
     if (in == out) return fail(KG_EINVAL, "kg_evolve: out must not alias in");
     if (!r_ok(R, true)) return fail(KG_EUNSUPPORTED, "R must be 1, 2, 4, 8 or 16");
@@ -1196,10 +1247,12 @@ extern "C" int kg_evolve(kg_hamiltonian *h, const kg_c128 *in, kg_c128 *out, int
     if ((rc = vec_in(h, WS_IN0, in, R, st, &din)) || (rc = vec_out(h, WS_OUT0, out, R, &o))) return rc;
     if ((rc = evolve_device(h, (const c128 *)din, R, (c128 *)o.dev, R, dt_fs, bessel_eps, st))) return rc;
     return vec_out_finish(h, o, st);
+    });
 }
 
 extern "C" int kg_apply_velocity(kg_hamiltonian *h, const kg_c128 *in, kg_c128 *out, int R, void *stream)
 {
+    return guarded([&]() -> int {
     if (!h || !in || !out) return fail(KG_EINVAL, "kg_apply_velocity: NULL argument");
     if (in == out) return fail(KG_EINVAL, "kg_apply_velocity: out must not alias in");
     if (!r_ok(R, true)) return fail(KG_EUNSUPPORTED, "R must be 1, 2, 4, 8 or 16");
@@ -1210,14 +1263,16 @@ extern "C" int kg_apply_velocity(kg_hamiltonian *h, const kg_c128 *in, kg_c128 *
     if ((rc = vec_in(h, WS_IN0, in, R, st, &din)) || (rc = vec_out(h, WS_OUT0, out, R, &o))) return rc;
     if ((rc = velocity_device(h, (const c128 *)din, R, (c128 *)o.dev, R, R, st))) return rc;
     return vec_out_finish(h, o, st);
+    });
 }
 
 extern "C" int kg_evolve_x(kg_hamiltonian *h, kg_c128 *psi, kg_c128 *psix, int R, double dt_fs,
                            double bessel_eps, void *stream)
 {
+    return guarded([&]() -> int {
     if (!h || !psi || !psix) return fail(KG_EINVAL, "kg_evolve_x: NULL argument");
     if (psi == psix) return fail(KG_EINVAL, "kg_evolve_x: psi and psix must be distinct");
-    if (!r_ok(R, false)) return fail(KG_EUNSUPPORTED, "R must be 1, 2, 4 or 8");
+    if (!r_ok(R, true)) return fail(KG_EUNSUPPORTED, "R must be 1, 2, 4, 8 or 16");
     if (!(dt_fs > 0.0) || !std::isfinite(dt_fs)) return fail(KG_EINVAL, "dt_fs must be finite and positive");
     cudaStream_t st = (cudaStream_t)stream;
     const size_t vbytes = (size_t)h->n * R * 16;
@@ -1245,12 +1300,15 @@ extern "C" int kg_evolve_x(kg_hamiltonian *h, kg_c128 *psi, kg_c128 *psix, int R
         if (src != user[q]) CUDA_TRY(cudaMemcpyAsync(user[q], src, vbytes, cudaMemcpyDefault, st));
     }
     return KG_OK;
+    });
 }
 
-static int check_corr_args(kg_hamiltonian *h, const void *phi, int R, int M, int n_steps, double dt_fs, void *mu)
+static int check_corr_args(kg_hamiltonian *h, const void *phi, int R, int M, int n_steps, double dt_fs, void *mu, bool allow16)
 {
     if (!h || !phi || !mu) return fail(KG_EINVAL, "NULL argument");
-    if (!r_ok(R, false)) return fail(KG_EUNSUPPORTED, "R must be 1, 2, 4 or 8");
+    if (!r_ok(R, allow16))
+        return fail(KG_EUNSUPPORTED, allow16 ? "R must be 1, 2, 4, 8 or 16"
+                                             : "R must be 1, 2, 4 or 8 (kg_vac advances a batch of 2R columns)");
     if (M < 2) return fail(KG_EINVAL, "M must be >= 2");
     if (n_steps < 0) return fail(KG_EINVAL, "n_steps must be >= 0");
     if (!(dt_fs > 0.0) || !std::isfinite(dt_fs)) return fail(KG_EINVAL, "dt_fs must be finite and positive");
@@ -1260,7 +1318,8 @@ static int check_corr_args(kg_hamiltonian *h, const void *phi, int R, int M, int
 extern "C" int kg_vac(kg_hamiltonian *h, const kg_c128 *phi, int R, int M, int n_steps, double dt_fs,
                       double bessel_eps, kg_c128 *mu, void *stream)
 {
-    int rc = check_corr_args(h, phi, R, M, n_steps, dt_fs, mu);
+    return guarded([&]() -> int {
+    int rc = check_corr_args(h, phi, R, M, n_steps, dt_fs, mu, false);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t vbytes = (size_t)h->n * R * 16;
@@ -1295,12 +1354,14 @@ extern "C" int kg_vac(kg_hamiltonian *h, const kg_c128 *phi, int R, int M, int n
         c128 *t = S; S = Sn; Sn = t;
     }
     return finish_out(o, st);
+    });
 }
 
 extern "C" int kg_msd(kg_hamiltonian *h, const kg_c128 *phi, int R, int M, int n_steps, double dt_fs,
                       double bessel_eps, kg_c128 *mu, void *stream)
 {
-    int rc = check_corr_args(h, phi, R, M, n_steps, dt_fs, mu);
+    return guarded([&]() -> int {
+    int rc = check_corr_args(h, phi, R, M, n_steps, dt_fs, mu, true);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t vbytes = (size_t)h->n * R * 16;
@@ -1326,6 +1387,7 @@ extern "C" int kg_msd(kg_hamiltonian *h, const kg_c128 *phi, int R, int M, int n
         t = X; X = Xn; Xn = t;
     }
     return finish_out(o, st);
+    });
 }
 
 // --------------------------------------------------------------------------------------
@@ -1335,6 +1397,7 @@ extern "C" int kg_kpm_reconstruct(const kg_c128 *mu, int64_t rows, int M, int ja
                                   double scale_eV, const double *energies_eV, int n_energies, double *f,
                                   void *stream)
 {
+    return guarded([&]() -> int {
     if (!mu || !energies_eV || !f) return fail(KG_EINVAL, "kg_kpm_reconstruct: NULL argument");
     if (rows <= 0 || rows > 65535 || M < 1 || n_energies < 1)
         return fail(KG_EINVAL, "kg_kpm_reconstruct: need 1 <= rows <= 65535, M >= 1, n_energies >= 1");
@@ -1363,6 +1426,7 @@ extern "C" int kg_kpm_reconstruct(const kg_c128 *mu, int64_t rows, int M, int ja
     CUDA_TRY(cudaGetLastError());
     if (!f_dev) CUDA_TRY(cudaMemcpyAsync(f, d_f, (size_t)rows * n_energies * 8, cudaMemcpyDeviceToHost, st));
     return KG_OK;
+    });
 }
 
 extern "C" int kg_transport(int n_steps, int n_energies, double dt_fs, double dens_per_nm2, double width_nm,
@@ -1370,6 +1434,7 @@ extern "C" int kg_transport(int n_steps, int n_energies, double dt_fs, double de
                             double *sigma_e1, double *sigma_e2, double *length_nm, double *conductance,
                             void *stream)
 {
+    return guarded([&]() -> int {
     if (n_steps < 0 || n_energies < 1) return fail(KG_EINVAL, "kg_transport: n_steps >= 0, n_energies >= 1");
     if (!(dt_fs > 0.0) || !std::isfinite(dt_fs) || !std::isfinite(dens_per_nm2) || !std::isfinite(width_nm))
         return fail(KG_EINVAL, "kg_transport: dt_fs must be positive; dens and width finite");
@@ -1401,6 +1466,7 @@ extern "C" int kg_transport(int n_steps, int n_energies, double dt_fs, double de
     for (int q = 0; q < 5; ++q)
         if (user[q] && dev[q] != user[q]) CUDA_TRY(cudaMemcpyAsync(user[q], dev[q], tbytes, cudaMemcpyDeviceToHost, st));
     return KG_OK;
+    });
 }
 
 // --------------------------------------------------------------------------------------
@@ -1414,7 +1480,8 @@ static int dot_device(kg_hamiltonian *h, const c128 *a, int ld_a, const c128 *b,
     case 2: kg_dot_kernel<2><<<grid, 256, 0, st>>>(a, ld_a, b, h->n, partial); break;
     case 4: kg_dot_kernel<4><<<grid, 256, 0, st>>>(a, ld_a, b, h->n, partial); break;
     case 8: kg_dot_kernel<8><<<grid, 256, 0, st>>>(a, ld_a, b, h->n, partial); break;
-    default: return fail(KG_EUNSUPPORTED, "R must be 1, 2, 4 or 8");
+    case 16: kg_dot_kernel<16><<<grid, 256, 0, st>>>(a, ld_a, b, h->n, partial); break;
+    default: return fail(KG_EUNSUPPORTED, "R must be 1, 2, 4, 8 or 16");
     }
     h->launches++;
     CUDA_TRY(cudaGetLastError());
@@ -1424,8 +1491,9 @@ static int dot_device(kg_hamiltonian *h, const c128 *a, int ld_a, const c128 *b,
 extern "C" int kg_fourier_moments(kg_hamiltonian *h, const kg_c128 *phiL, const kg_c128 *phiR, int R, int Nm,
                                   double dtau_fs, double bessel_eps, kg_c128 *F, void *stream)
 {
+    return guarded([&]() -> int {
     if (!h || !phiL || !phiR || !F) return fail(KG_EINVAL, "kg_fourier_moments: NULL argument");
-    if (!r_ok(R, false)) return fail(KG_EUNSUPPORTED, "R must be 1, 2, 4 or 8");
+    if (!r_ok(R, true)) return fail(KG_EUNSUPPORTED, "R must be 1, 2, 4, 8 or 16");
     if (Nm < 0) return fail(KG_EINVAL, "Nm must be >= 0");
     if (!(dtau_fs > 0.0) || !std::isfinite(dtau_fs)) return fail(KG_EINVAL, "dtau_fs must be finite and positive");
     cudaStream_t st = (cudaStream_t)stream;
@@ -1461,11 +1529,13 @@ extern "C" int kg_fourier_moments(kg_hamiltonian *h, const kg_c128 *phiL, const 
     h->launches++;
     CUDA_TRY(cudaGetLastError());
     return finish_out(o, st);
+    });
 }
 
 extern "C" int kg_ftm_reconstruct(const kg_c128 *F, int64_t rows, int Nm, int window, double dtau_fs,
                                   const double *energies_eV, int n_energies, double *f, void *stream)
 {
+    return guarded([&]() -> int {
     if (!F || !energies_eV || !f) return fail(KG_EINVAL, "kg_ftm_reconstruct: NULL argument");
     if (rows <= 0 || rows > 65535 || Nm < 0 || n_energies < 1)
         return fail(KG_EINVAL, "kg_ftm_reconstruct: need 1 <= rows <= 65535, Nm >= 0, n_energies >= 1");
@@ -1486,4 +1556,5 @@ extern "C" int kg_ftm_reconstruct(const kg_c128 *F, int64_t rows, int Nm, int wi
     CUDA_TRY(cudaGetLastError());
     if (!f_dev) CUDA_TRY(cudaMemcpyAsync(f, d_f, (size_t)rows * n_energies * 8, cudaMemcpyDeviceToHost, st));
     return KG_OK;
+    });
 }

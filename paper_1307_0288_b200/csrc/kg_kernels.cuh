@@ -259,6 +259,15 @@ __global__ void kg_build_matrix(int64_t n, int64_t ns, int kmax, const int32_t *
     atomicMax(gersh, (unsigned long long)__double_as_longlong(gmax));
 }
 
+// flag |= 1 if any of the `count` doubles is NaN or Inf (KG_OPT_CHECK_INPUT)
+__global__ void kg_check_finite(const double *__restrict__ v, int64_t count, unsigned int *flag)
+{
+    bool bad = false;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < count; e += (int64_t)gridDim.x * blockDim.x)
+        bad |= !isfinite(v[e]);
+    if (bad) atomicOr(flag, 1u);
+}
+
 // dst[i*R + r] = src[map[i]*R + r]: caller order -> internal order with map = perm, and back with
 // map = iperm (one thread per element, coalesced writes, 16-byte gathers)
 __global__ void kg_permute_rows(const c128 *__restrict__ src, c128 *__restrict__ dst,
@@ -347,7 +356,9 @@ __global__ void kg_kpm_reconstruct_kernel(const c128 *__restrict__ mu, int64_t r
         const double t2 = fma(2.0 * x, t1, -t0);
         t0 = t1; t1 = t2;
     }
-    f[row * (int64_t)ne + j] = sum / (3.14159265358979323846 * s * sqrt(1.0 - x * x));
+    // outside (-1, 1) the reconstruction is undefined: NaN (a device grid is not validated on the host)
+    f[row * (int64_t)ne + j] = fabs(x) < 1.0 ? sum / (3.14159265358979323846 * s * sqrt(1.0 - x * x))
+                                             : __longlong_as_double(0x7ff8000000000000LL);
 }
 
 // ---------------------------------------------------------------------------------------

@@ -687,3 +687,35 @@ def test_zgnr_first_plateau_conductance(kgo):
     assert 2 * np.sqrt(np.max(fmsd[-1] / rho)) < 0.45 * lat.period_x       # the wave packet has not wrapped around
     print("ZGNR first plateau G/(2e^2/h) at t_k, k = 6, 9, 12:", np.round(g[[6, 9, 12]], 4))
     assert np.max(np.abs(g[6:] - 1.0)) < 0.05
+
+
+# ------------------------------------------------------------------ local density of states
+def test_ldos_vacancy_zero_mode(kgo):
+    """Local DOS from unit vectors on 8 x 8 cells with ONE vacancy (255 sites).  Textbook: on a
+    bipartite lattice with N_B = N_A + 1 there is exactly one zero-energy state and it lives on the
+    majority sublattice.  The oracle's moments for |i> equal sum_j |<j|i>|^2 T_n(E_j/s) from the dense
+    spectrum, and the weight of its KPM local DOS around E = 0 is the zero mode's |<0|i>|^2: large on a
+    neighbour of the vacancy, exactly zero on the minority sublattice."""
+    full = kgo.honeycomb(8, 8)
+    vac = np.zeros(full.n, np.uint8); vac[4 * (3 * 8 + 3) + 0] = 1            # one A-type site (basis b0)
+    lat = kgo.remove_sites(full, vac)
+    _, E, Vec = eig(lat)
+    assert np.sum(np.abs(E) < 1e-9) == 1
+    zero = Vec[:, np.argmin(np.abs(E))]
+    gap = np.sort(np.abs(E))[1]
+    assert gap > 0.3                                                          # the finite sheet's other levels are far away
+    s, M = S_GRAPHENE, 600                                                    # Jackson width pi s / M = 0.045 eV << gap
+    nbr = int(np.argmax(np.abs(zero)))                                        # strongest site: next to the vacancy
+    assert lat.nn[nbr] == 2
+    # a site of the minority sublattice: bipartite => the zero mode vanishes there
+    minority = [i for i in range(lat.n) if abs(zero[i]) < 1e-12]
+    assert len(minority) == 127
+    en = np.linspace(-0.25, 0.25, 501)
+    for site, w in ((nbr, zero[nbr] ** 2), (minority[5], 0.0)):
+        phi = np.zeros(lat.n, complex); phi[site] = 1.0
+        mu = kgo.dos_moments(lat, 0.0, s, phi, M)
+        want = np.array([np.sum(Vec[site] ** 2 * cheb_T(m, E / s)) for m in range(M)])
+        assert relerr(mu, want) < 1e-12
+        weight = np.trapezoid(kgo.kpm_reconstruct(mu, 0.0, s, en), en)
+        assert abs(weight - w) < 2e-3
+    assert zero[nbr] ** 2 > 0.1
