@@ -104,6 +104,53 @@ void kgo_honeycomb(int64_t ncx, int64_t ncy, int periodic_x, int periodic_y, dou
             }
 }
 
+/* Honeycomb sheet with next-nearest-neighbour hopping ("more complicated tight-binding  */
+/* models ... denser Hamiltonian"; the t' term of the standard graphene model): row width 9 — the */
+/* three nearest neighbours of kgo_honeycomb in the same order with hopping t, then the six         */
+/* second neighbours at distance sqrt(3) a (same sublattice) with hopping t2, in the order          */
+/* (+2,0) (-2,0) (+1,+3) (-1,+3) (+1,-3) (-1,-3) of displacements in units (h, a/2).  Offsets wrap   */
+/* on periodic axes, otherwise the neighbour is dropped and later ones shift down.  Outputs sized  */
+/* for kmax = 9: nl[k*n+i], hop[k*n+i]; unused slots hold i and 0.                                  */
+static const int NB2[4][6][3] = {   /* (dcx, dcy, b') for the six second neighbours of basis b */
+    {{1, 0, 0}, {-1, 0, 0}, {0, 0, 2}, {-1, 0, 2}, {0, -1, 2}, {-1, -1, 2}},
+    {{1, 0, 1}, {-1, 0, 1}, {0, 0, 3}, {-1, 0, 3}, {0, -1, 3}, {-1, -1, 3}},
+    {{1, 0, 2}, {-1, 0, 2}, {1, 1, 0}, {0, 1, 0}, {1, 0, 0}, {0, 0, 0}},
+    {{1, 0, 3}, {-1, 0, 3}, {1, 1, 1}, {0, 1, 1}, {1, 0, 1}, {0, 0, 1}},
+};
+
+void kgo_honeycomb_nnn(int64_t ncx, int64_t ncy, int periodic_x, int periodic_y, double a_nm, double t_eV,
+                       double t2_eV, double *x, double *y, int32_t *nn, int32_t *nl, double *hop)
+{
+    const int64_t n = 4 * ncx * ncy;
+    const double h = sqrt(3.0) * a_nm / 2.0;
+    const double q = a_nm / 2.0;
+    for (int64_t cy = 0; cy < ncy; ++cy)
+        for (int64_t cx = 0; cx < ncx; ++cx)
+            for (int b = 0; b < 4; ++b) {
+                const int64_t i = 4 * (cy * ncx + cx) + b;
+                x[i] = (double)(2 * cx + HX[b]) * h;
+                y[i] = (double)(6 * cy + HY[b]) * q;
+                int cnt = 0;
+                for (int k = 0; k < 9; ++k) {
+                    const int *e = k < 3 ? NB[b][k] : NB2[b][k - 3];
+                    int64_t mx = cx + e[0], my = cy + e[1];
+                    if (mx < 0 || mx >= ncx) {
+                        if (!periodic_x) continue;
+                        mx = (mx + ncx) % ncx;
+                    }
+                    if (my < 0 || my >= ncy) {
+                        if (!periodic_y) continue;
+                        my = (my + ncy) % ncy;
+                    }
+                    nl[(int64_t)cnt * n + i] = (int32_t)(4 * (my * ncx + mx) + e[2]);
+                    hop[(int64_t)cnt * n + i] = k < 3 ? t_eV : t2_eV;
+                    ++cnt;
+                }
+                nn[i] = cnt;
+                for (int k = cnt; k < 9; ++k) { nl[(int64_t)k * n + i] = (int32_t)i; hop[(int64_t)k * n + i] = 0.0; }
+            }
+}
+
 /* Vacancies ("removing carbon atoms randomly"; reading g15: delete and  */
 /* compact).  The vacant set is the n_vac sites with the smallest (key, index) */
 /* pairs, key_j = mix64(seed, stream 0, j).  vacant[j] = 1 if removed.         */

@@ -97,6 +97,19 @@ def honeycomb(ncx, ncy, periodic_x=True, periodic_y=True, a_nm=0.142, t_eV=-2.7)
     return Lattice(n, 3, nn, nl, hop, None, x, y, px, py)
 
 
+def honeycomb_nnn(ncx, ncy, periodic_x=True, periodic_y=True, a_nm=0.142, t_eV=-2.7, t2_eV=-0.27):
+    """Honeycomb sheet with nearest (t) and next-nearest (t2) neighbour hopping, row width 9."""
+    n = 4 * ncx * ncy
+    x = np.empty(n); y = np.empty(n)
+    nn = np.empty(n, np.int32); nl = np.empty(9 * n, np.int32); hop = np.empty(9 * n)
+    lib().kgo_honeycomb_nnn(C.c_int64(ncx), C.c_int64(ncy), C.c_int(int(periodic_x)), C.c_int(int(periodic_y)),
+                            C.c_double(a_nm), C.c_double(t_eV), C.c_double(t2_eV), _p(x), _p(y), _p(nn), _p(nl), _p(hop))
+    h = np.sqrt(3.0) * a_nm / 2.0
+    px = 2 * ncx * h if periodic_x else 0.0
+    py = 6 * ncy * (a_nm / 2.0) if periodic_y else 0.0
+    return Lattice(n, 9, nn, nl, hop, None, x, y, px, py)
+
+
 def hop_from_nn(nn, t_eV):
     """hop[k*n+i] = t for k < nn[i], 0 for unused slots (ELL padding)."""
     n = nn.shape[0]

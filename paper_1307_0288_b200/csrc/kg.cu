@@ -310,6 +310,7 @@ static cudaError_t staged_launch(kg_hamiltonian *h, int mode, int R, const Stage
     case 3: return kg_staged_launch_k3(mode, R, a, l, st);
     case 4: return kg_staged_launch_k4(mode, R, a, l, st);
     case 6: return kg_staged_launch_k6(mode, R, a, l, st);
+    case 9: return kg_staged_launch_k9(mode, R, a, l, st);
     }
     return cudaErrorInvalidValue;
 }

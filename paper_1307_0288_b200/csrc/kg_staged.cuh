@@ -116,7 +116,7 @@ __host__ __device__ constexpr int sg_stage_bytes(int R, int K, int mode, bool on
             (sg_is_pair(mode) ? 8 * K : 0) + (dict ? 0 : 8 * K)) + 127) / 128 * 128;
 }
 // row widths the staged kernels are compiled for (others run kg_step_kernel)
-__host__ __device__ constexpr bool sg_k_supported(int K) { return K == 2 || K == 3 || K == 4 || K == 6; }
+__host__ __device__ constexpr bool sg_k_supported(int K) { return K == 2 || K == 3 || K == 4 || K == 6 || K == 9; }
 __host__ __device__ constexpr int sg_header_bytes(int R)
 {
     return (2 * SG_MAX_STAGES * 8 + 16 * 8 + 32 * R * 16 + 127) / 128 * 128;

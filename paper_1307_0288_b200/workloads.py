@@ -108,15 +108,69 @@ def honeycomb(ncx: int, ncy: int, periodic_x=True, periodic_y=True, a_nm=A_NM, t
                    {"ncx": ncx, "ncy": ncy})
 
 
-def _pack_neighbours(cand, valid, n):
-    """Shift valid neighbours down to slots 0..nn-1 keeping their order; pad with self."""
+def _pack_neighbours(cand, valid, n, values=None):
+    """Shift valid neighbours down to slots 0..nn-1 keeping their order; pad with self (and 0 in the
+    optional per-slot values, which are packed the same way)."""
+    kmax = cand.shape[0]
     nn = valid.sum(axis=0).astype(np.int32)
     slot = np.cumsum(valid, axis=0) - 1            # target slot of each valid candidate
-    nl = np.tile(np.arange(n, dtype=np.int64), (3, 1))
-    for k in range(3):
+    nl = np.tile(np.arange(n, dtype=np.int64), (kmax, 1))
+    vals = None if values is None else np.zeros((kmax, n))
+    for k in range(kmax):
         sel = valid[k]
         nl[slot[k, sel], np.nonzero(sel)[0]] = cand[k, sel]
-    return nn, nl.astype(np.int32).reshape(3 * n)
+        if values is not None:
+            vals[slot[k, sel], np.nonzero(sel)[0]] = values[k]
+    if values is None:
+        return nn, nl.astype(np.int32).reshape(kmax * n)
+    return nn, nl.astype(np.int32).reshape(kmax * n), vals.reshape(kmax * n)
+
+
+T2_EV = -0.27         # next-nearest-neighbour hopping t' = 0.1 |t| (graphene: 0.02-0.2 |t| in the literature)
+
+
+def honeycomb_nnn(ncx: int, ncy: int, periodic_x=True, periodic_y=True, a_nm=A_NM, t_eV=T_EV, t2_eV=T2_EV) -> Lattice:
+    """Honeycomb sheet with next-nearest-neighbour hopping (a "more complicated tight-binding
+    model" with a denser Hamiltonian): row width 9 — the three nearest neighbours of `honeycomb` in the
+    same order (hopping t), then the six second neighbours at distance sqrt(3) a (hopping t2) in the
+    order (+2,0) (-2,0) (+1,+3) (-1,+3) (+1,-3) (-1,-3) of displacements in units (h, a/2)."""
+    n = 4 * ncx * ncy
+    site = np.arange(n, dtype=np.int64)
+    b = site & 3
+    cell = site >> 2
+    cx = cell % ncx
+    cy = cell // ncx
+    h = np.sqrt(3.0) * a_nm / 2.0
+    q = a_nm / 2.0
+    x = (2 * cx + np.where(b >= 2, 1, 0)).astype(np.float64) * h
+    y = (6 * cy + np.array([0, 2, 3, 5], dtype=np.int64)[b]).astype(np.float64) * q
+    # (dcx, dcy, basis') per basis b and neighbour k: three nearest, six second neighbours
+    tab = np.array([
+        [(0, 0, 1), (0, -1, 3), (-1, -1, 3), (1, 0, 0), (-1, 0, 0), (0, 0, 2), (-1, 0, 2), (0, -1, 2), (-1, -1, 2)],
+        [(0, 0, 0), (0, 0, 2), (-1, 0, 2), (1, 0, 1), (-1, 0, 1), (0, 0, 3), (-1, 0, 3), (0, -1, 3), (-1, -1, 3)],
+        [(0, 0, 3), (0, 0, 1), (1, 0, 1), (1, 0, 2), (-1, 0, 2), (1, 1, 0), (0, 1, 0), (1, 0, 0), (0, 0, 0)],
+        [(0, 0, 2), (0, 1, 0), (1, 1, 0), (1, 0, 3), (-1, 0, 3), (1, 1, 1), (0, 1, 1), (1, 0, 1), (0, 0, 1)],
+    ], dtype=np.int64)
+    cand = np.empty((9, n), dtype=np.int64)
+    valid = np.ones((9, n), dtype=bool)
+    for k in range(9):
+        mx = cx + tab[b, k, 0]
+        my = cy + tab[b, k, 1]
+        okx = (mx >= 0) & (mx < ncx)
+        oky = (my >= 0) & (my < ncy)
+        if periodic_x:
+            mx = np.mod(mx, ncx)
+        else:
+            valid[k] &= okx
+        if periodic_y:
+            my = np.mod(my, ncy)
+        else:
+            valid[k] &= oky
+        cand[k] = 4 * (np.clip(my, 0, ncy - 1) * ncx + np.clip(mx, 0, ncx - 1)) + tab[b, k, 2]
+    nn, nl, hop = _pack_neighbours(cand, valid, n, values=[t_eV] * 3 + [t2_eV] * 6)
+    return Lattice(n, 9, nn, nl, hop, None, x, y,
+                   2 * ncx * h if periodic_x else 0.0, 6 * ncy * q if periodic_y else 0.0,
+                   {"ncx": ncx, "ncy": ncy, "t2_eV": t2_eV})
 
 
 def _hop_from_nn(nn, t_eV):

@@ -181,3 +181,32 @@ def test_zgnr_config_counts():
     cfg = W.make_config(6, shrink=64)
     assert cfg.lattice.n == 1_048_576 // 64 and cfg.R == 1 and cfg.M == 2000
     assert abs(cfg.period - 65536 // 64 * np.sqrt(3.0) * 0.142 / 2) < 1e-9      # L_x = sqrt(3) N_x a / 2
+
+
+@pytest.mark.parametrize("args", [(5, 4, True, True), (6, 3, False, True), (3, 5, True, False), (4, 4, False, False)])
+def test_honeycomb_nnn_bit_exact(kgo, args):
+    """Next-nearest-neighbour sheet (row width 9, two hopping values): the two generators agree bit for
+    bit; on the torus every site has 3 first neighbours at distance a and 6 second neighbours at sqrt(3) a
+    on its own sublattice; the adjacency is symmetric with equal hoppings both ways."""
+    a, b = kgo.honeycomb_nnn(*args), W.honeycomb_nnn(*args)
+    for f in ("nn", "nl", "hop", "x", "y"):
+        assert np.array_equal(getattr(a, f), getattr(b, f)), f
+    assert b.kmax == 9
+    nl, hop = b.nl.reshape(9, b.n), b.hop.reshape(9, b.n)
+    i = np.broadcast_to(np.arange(b.n), (9, b.n))
+    valid = np.arange(9)[:, None] < b.nn[None, :]
+    dx, dy = b.x[nl] - b.x[i], b.y[nl] - b.y[i]
+    if b.period_x > 0:
+        dx -= b.period_x * np.round(dx / b.period_x)
+    if b.period_y > 0:
+        dy -= b.period_y * np.round(dy / b.period_y)
+    dist = np.hypot(dx, dy)
+    first, second = valid & (hop == -2.7), valid & (hop == -0.27)
+    assert np.all(first | second == valid)
+    assert np.max(np.abs(dist[first] - 0.142)) < 1e-12 and np.max(np.abs(dist[second] - np.sqrt(3) * 0.142)) < 1e-12
+    sub = (np.arange(b.n) & 1)                                   # b0, b2 on one sublattice, b1, b3 on the other
+    assert np.all(sub[nl][first] != sub[i][first]) and np.all(sub[nl][second] == sub[i][second])
+    if args[2] and args[3]:
+        assert np.all(b.nn == 9) and np.all(first.sum(axis=0) == 3) and np.all(second.sum(axis=0) == 6)
+    pairs = {(int(p), int(m)): float(v) for p, m, v in zip(i[valid], nl[valid], hop[valid])}
+    assert all(pairs.get((m, p)) == v for (p, m), v in pairs.items())

@@ -719,3 +719,33 @@ def test_ldos_vacancy_zero_mode(kgo):
         weight = np.trapezoid(kgo.kpm_reconstruct(mu, 0.0, s, en), en)
         assert abs(weight - w) < 2e-3
     assert zero[nbr] ** 2 > 0.1
+
+
+# ------------------------------------------------------------------ next-nearest-neighbour model
+def test_nnn_graphene_bands(kgo):
+    """Denser Hamiltonian (row width 9): the dense spectrum of the generated next-nearest-neighbour torus
+    equals the textbook bands E(k) = t' f(k) +- |t| sqrt(3 + f(k)), f = 2 [cos k.a1 + cos k.a2 + cos k.(a2-a1)]
+    (Wallace 1947; Castro Neto et al. RMP 2009 eq 6) on the allowed k, and the oracle's full-trace moments with
+    E0 = 3 t' != 0 (the Dirac-point energy) equal the moments of that spectrum."""
+    ncx, ncy, t, t2 = 6, 4, -2.7, -0.27
+    lat = kgo.honeycomb_nnn(ncx, ncy, t_eV=t, t2_eV=t2)
+    _, E, _ = eig(lat)
+    h = np.sqrt(3) * A / 2
+    a1, a2 = np.array([2 * h, 0.0]), np.array([h, 1.5 * A])
+    vals = []
+    for p in range(ncx):
+        for q in range(ncy):
+            for bz in range(2):
+                k = np.array([2 * np.pi * p / (ncx * 2 * h), 2 * np.pi * q / (ncy * 3 * A) + bz * 2 * np.pi / (3 * A)])
+                f = 2 * (np.cos(k @ a1) + np.cos(k @ a2) + np.cos(k @ (a2 - a1)))
+                root = abs(t) * np.sqrt(max(3 + f, 0.0))
+                vals += [t2 * f + root, t2 * f - root]
+    assert np.max(np.abs(np.sort(vals) - E)) < 1e-12
+    e0 = -3 * t2                                                  # Dirac point of this sign convention
+    s = (abs(e0) + 3 * abs(t) + 6 * abs(t2)) * 1.05
+    M = 40
+    mu = np.zeros(M)
+    for i in range(lat.n):
+        phi = np.zeros(lat.n, complex); phi[i] = 1.0
+        mu += kgo.dos_moments(lat, e0, s, phi, M).real
+    assert relerr(mu / lat.n, np.array([np.mean(cheb_T(m, (E - e0) / s)) for m in range(M)])) < 1e-12
