@@ -280,6 +280,11 @@ enum {
     KG_OPT_CHECK_INPUT = 14, /* 1: every input vector is scanned for NaN / Inf (one extra pass and a stream
                                 synchronisation per call) and the call returns KG_EINVAL; 0 (default): not checked —
                                 non-finite input gives non-finite output.  (The matrix is always checked at create.) */
+    KG_OPT_ONE_LAUNCH = 15,  /* launch-bound sizes (all 512-element tiles of a batch fit the shared memory of one
+                                8-CTA cluster: n * R <= 16 K elements for the paper's model): the moment loop after
+                                its first step runs as ONE kernel, one cluster barrier per Chebyshev step, vectors
+                                and matrix rows in distributed shared memory; bitwise equal to the per-step
+                                launches.  -1 (default) / 1: on when eligible, 0: off */
     KG_OPT_PDL = 11          /* consecutive sweeps chained by programmatic dependent launch (the next sweep's
                                 CTAs are scheduled while this one drains): 1 on, 0 off, -1 (default) on for
                                 launch-bound sizes, n * R <= 2^18 */

@@ -32,6 +32,7 @@ KG_OPT_PDL = 11
 KG_OPT_REORDER = 12
 KG_OPT_TWO_STEP = 13
 KG_OPT_CHECK_INPUT = 14
+KG_OPT_ONE_LAUNCH = 15
 
 _vp, _i64, _i32, _dbl, _int = C.c_void_p, C.c_int64, C.c_int32, C.c_double, C.c_int
 _lib.kg_last_error.restype = C.c_char_p

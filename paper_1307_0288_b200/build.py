@@ -1,6 +1,6 @@
 """In-tree build of libkg.so (CUDA, sm_100a) with nvcc.  `python -m paper_1307_0288_b200.build`.
 
-The library is seven translation units — kg.cu (C ABI, drivers, one-thread-per-element kernels)
+The library is eight translation units — kg.cu (C ABI, drivers, one-thread-per-element kernels)
 one kg_staged_k<K>.cu per compiled neighbour-list row width and kg_tb2.cu (two-step kernels) — compiled in parallel and linked
 with the CUDA runtime statically (no libtorch)."""
 from __future__ import annotations
@@ -14,10 +14,10 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 SRC = [os.path.join(CSRC, f) for f in ("kg.cu", "kg_staged_k2.cu", "kg_staged_k3.cu", "kg_staged_k4.cu",
-                                       "kg_staged_k6.cu", "kg_staged_k9.cu", "kg_tb2.cu")]
+                                       "kg_staged_k6.cu", "kg_staged_k9.cu", "kg_tb2.cu", "kg_small.cu")]
 HEADERS = [os.path.join(CSRC, f) for f in ("kg_common.cuh", "kg_kernels.cuh", "kg_staged.cuh",
                                            "kg_staged_impl.cuh", "kg_staged_launch.h", "kg_partition.h",
-                                           "kg_tb2.cuh", "kg_tb2_launch.h")]
+                                           "kg_tb2.cuh", "kg_tb2_launch.h", "kg_small.cuh", "kg_small_launch.h")]
 DEPS = SRC + HEADERS + [os.path.join(ROOT, "include", "kg.h")]
 LIB = os.path.join(HERE, "libkg.so")
 OBJ_DIR = os.path.join(HERE, "build")

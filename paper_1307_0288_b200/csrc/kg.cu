@@ -8,6 +8,8 @@
 #include "kg_partition.h"
 #include "kg_tb2.cuh"
 #include "kg_tb2_launch.h"
+#include "kg_small.cuh"
+#include "kg_small_launch.h"
 
 #include <algorithm>
 #include <cmath>
@@ -116,6 +118,7 @@ struct kg_hamiltonian {
     int ndict;                // entries in use (0: hoppings do not fit a dictionary)
     int staged, stages, staged_ctas, alternate, doubling, clenshaw, pdl;   // options of the staged kernel
     int tb2;                  // KG_OPT_TWO_STEP: -1 auto, 0 off, 1 whenever a plan exists
+    int one_launch;           // KG_OPT_ONE_LAUNCH: -1 auto, 0 off: the moment loop of launch-bound sizes as one cluster kernel
     int check_input;          // KG_OPT_CHECK_INPUT: input vectors are scanned for NaN / Inf (one pass + a synchronisation)
     unsigned int *d_flag;     // device flag of that scan
     Tb2Plan tbp[2];
@@ -581,7 +584,7 @@ static int create_from_device_list(kg_hamiltonian **out, int64_t n, int kmax, co
     h->nl = h->nlp = nullptr; h->hop = h->xhop = h->onsite = nullptr;
     h->perm = h->iperm = nullptr;
     h->tb2 = -1; memset(h->tbp, 0, sizeof(h->tbp));
-    h->check_input = 0; h->d_flag = nullptr;
+    h->check_input = 0; h->d_flag = nullptr; h->one_launch = -1;
     h->ndict = 0; h->staged = 1; h->stages = 0; h->staged_ctas = 0; h->alternate = 1; h->doubling = 1; h->clenshaw = 1; h->pdl = -1;
     memset(h->dict, 0, sizeof(h->dict));
     memset(h->ws, 0, sizeof(h->ws));
@@ -870,6 +873,7 @@ extern "C" int kg_set_option(kg_hamiltonian *h, int option, int64_t value)
     case KG_OPT_PDL: h->pdl = value < 0 ? -1 : (value != 0); break;
     case KG_OPT_TWO_STEP: h->tb2 = value < 0 ? -1 : (value != 0); break;
     case KG_OPT_CHECK_INPUT: h->check_input = value != 0; break;
+    case KG_OPT_ONE_LAUNCH: h->one_launch = value < 0 ? -1 : (value != 0); break;
     case KG_OPT_DICT:
         if (value != 0) return fail(KG_EINVAL, "the dictionary can only be switched off");
         h->ndict = 0; break;
@@ -994,6 +998,31 @@ static int moments_device(kg_hamiltonian *h, const c128 *phiL, int ldL, const c1
                 if (old_prev != phiR) freeb.push_back(old_prev);
             }
             m += nstep;
+        }
+    } else if (h->one_launch != 0 && sp.ok && sp.grid == sp.ntiles && ldL == R && ldR == R && R <= 8 && h->kmax <= 12 &&
+               (sp.ntiles + SM_MAX_CLUSTER - 1) / SM_MAX_CLUSTER <= 255 &&
+               (sp.ntiles + SM_MAX_CLUSTER - 1) / SM_MAX_CLUSTER * sm_tile_bytes(R, h->kmax, mode == MODE_MOM) <= (size_t)200 * 1024) {
+        // launch-bound sizes: first step, then ALL further steps in one cluster kernel whose CTAs keep their
+        // tiles in (distributed) shared memory (kg_small.cuh); bitwise equal to the one-launch-per-step path
+        const size_t prow = (size_t)grid * PR;
+        c128 *P = (c128 *)part;
+        StepArgs a = base_args(h);
+        a.phiL = phiL; a.ld_L = ldL; a.alpha = 1.0;
+        a.cur = phiR; a.ld_cur = ldR; a.next = (c128 *)ta;
+        a.partial0 = P; a.partial = P + prow; a.partial2 = P + 2 * prow;
+        CUDA_TRY(launch_step(h, mode, true, R, a, grid, st));
+        const int m_end = dbl ? M / 2 + 1 : M;
+        if (m_end > 2) {
+            SmallArgs sa;
+            memset(&sa, 0, sizeof(sa));
+            sa.nl = h->nl; sa.hop = h->hop; sa.onsite = h->onsite; sa.n = h->n; sa.ns = h->ns; sa.K = h->kmax;
+            sa.ons = h->has_onsite ? 1 : 0;
+            sa.t0 = phiR; sa.t1 = (const c128 *)ta; sa.phiL = phiL; sa.part = P; sa.m_end = m_end;
+            sa.ntiles = sp.ntiles; sa.vt = (sp.ntiles + SM_MAX_CLUSTER - 1) / SM_MAX_CLUSTER;
+            sa.alternate = h->alternate;
+            const int ncta = (sp.ntiles + sa.vt - 1) / sa.vt;
+            h->launches++;
+            CUDA_TRY(kg_small_launch(mode, R, sa, ncta, (size_t)sa.vt * sm_tile_bytes(R, h->kmax, mode == MODE_MOM), h->device, st));
         }
     } else if (want_graph(h, elems, st)) {
         cudaGraphExec_t exec = nullptr;
