@@ -74,6 +74,7 @@ def test_staged_moments_hopping_kinds(B, kgo, R, kind, onsite):
     rng = np.random.default_rng(R)
     L = rng.normal(size=(lat.n, R)) + 1j * rng.normal(size=(lat.n, R))
     M = 80
+    h.set_option(B.KG_OPT_ONE_LAUNCH, 0)   # one launch per step here (the single-launch loop: tests/test_gpu_small.py)
     launches0 = h.launch_count
     mu = host(B.moments(h, dev(L), dev(phi), M))
     for r in range(R):
@@ -199,6 +200,7 @@ def test_doubling_moments(B, kgo, M, R, staged):
     olat = to_oracle_lattice(kgo, lat)
     h = B.from_lattice(lat, lat.x, lat.period_x, 0.0, s)
     h.set_option(B.KG_OPT_STAGED, staged)
+    h.set_option(B.KG_OPT_ONE_LAUNCH, 0)   # count the per-step launches (single-launch loop: tests/test_gpu_small.py)
     rng = np.random.default_rng(M)
     phi = rng.normal(size=(lat.n, R)) + 1j * rng.normal(size=(lat.n, R))     # not normalised
     d = dev(phi)
