@@ -341,6 +341,8 @@ def run_b200(args, cfg):
         bdef = ("must-move bytes of the launched one-step sweep: (48 + (4 K + 8)/C) B per site-update (T_m, T_m-1 read, T_m+1 "
                 "written, packed index + on-site row shared by the C columns)")
         tkey = f"{cfg.name}_momx_R{C}"
+    if sweeps == 1 and steps > 2:
+        kname = "kg_small_kernel (launch-bound size: all Chebyshev steps after the first in ONE cluster launch, vectors in distributed shared memory)"
     steps_per_launch = steps / sweeps if sweeps > 0 else 1.0
     updates_launch = n * C * steps_per_launch
     bytes_8d = mom_bytes_per_update(C, lat.kmax, phi_l_stream=False) * updates_launch
@@ -358,6 +360,27 @@ def run_b200(args, cfg):
                                                   "fraction exceeds 1 — the roofline fraction is `frac`, on the bytes really required"},
                 "us_per_launch": kern_us,
                 "gsu_per_s": updates_launch / (kern_us * 1e-6) / 1e9, "traffic": ncu_traffic(tkey)}
+
+    # second kernel of the step (about 40 %): the DOS / MSD moment sweep on one column, kg_dos_moments(M) =
+    # first step + passes + reduction, timed the same way
+    l0 = h.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(reps):
+        B.dos_moments(h, phi_dev, M, mu=mu_dos)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    sweeps1 = (h.launch_count - l0) // reps - 2                 # minus first step, reduction
+    us1 = e0.elapsed_time(e1) * 1e3 / (reps * (sweeps1 + 1))
+    spl1 = steps / sweeps1 if sweeps1 > 0 else 1.0
+    bytes1 = ((64.0 * R + 8.0 + (8.0 if ons else 0.0)) * n) if sweeps1 < steps else must_move_bytes_per_update(R, lat.kmax, ons) * n * R
+    roofline["second_kernel"] = {
+        "kernel": ("kg_small_kernel" if (sweeps1 == 1 and steps > 2) else f"kg_tb2_kernel<C={R}, K={lat.kmax}, MODE_MOM2, NSTEP=2>" if sweeps1 < steps else f"kg_staged_kernel<R={R}, MODE_MOM2>") +
+                  " (DOS / MSD moment sweeps, phi_L = phi_R)",
+        "us_per_launch": us1, "chebyshev_steps_per_launch": spl1, "bytes_per_launch": bytes1,
+        "achieved": bytes1 / (us1 * 1e-6) / 1e9, "frac": bytes1 / (us1 * 1e-6) / 1e9 / peak,
+        "gsu_per_s": n * R * spl1 / (us1 * 1e-6) / 1e9,
+        "traffic": ncu_traffic(f"{cfg.name}_tb2_mom2_C{R}" if sweeps1 < steps else f"{cfg.name}_mom2_R{R}")}
 
     if rank != 0:
         ctx.finalize()

@@ -61,7 +61,12 @@ extern "C" const char *kg_last_error(void) { return g_err; }
 // options read by kg_create_hamiltonian[_csr] (set before create; process-wide)
 static int g_reorder = -1;                    // KG_OPT_REORDER: -1 auto, 0 off, 1 always
 #define KG_REORDER_MIN_SITES ((int64_t)1 << 16)
+#ifndef KG_REORDER_GROUP
+#define KG_REORDER_GROUP 8           // consecutive caller sites that stay together (kg_partition.h)
+#endif
+#ifndef KG_REORDER_LEAF
 #define KG_REORDER_LEAF 64
+#endif
 
 extern "C" int kg_set_default_option(int option, int64_t value)
 {
@@ -614,7 +619,7 @@ static int create_from_device_list(kg_hamiltonian **out, int64_t n, int kmax, co
             (e = cudaMemcpyAsync(h_nl.data(), d_nl, (size_t)n * kmax * 4, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
             (e = cudaStreamSynchronize(st)) != cudaSuccess)
             return cleanup(fail(KG_ECUDA, "neighbour list to host: %s", cudaGetErrorString(e)));
-        kg_partition_host(n, kmax, h_nn.data(), h_nl.data(), KG_REORDER_LEAF, perm);
+        kg_partition_grouped(n, kmax, h_nn.data(), h_nl.data(), KG_REORDER_LEAF, KG_REORDER_GROUP, perm);
         for (int64_t i = 0; i < n; ++i) iperm[(size_t)perm[(size_t)i]] = (int32_t)i;
         if ((e = cudaMalloc(&h->perm, (size_t)n * 4)) != cudaSuccess || (e = cudaMalloc(&h->iperm, (size_t)n * 4)) != cudaSuccess)
             return cleanup(fail(KG_ENOMEM, "permutation allocation: %s", cudaGetErrorString(e)));

@@ -87,3 +87,55 @@ static inline void kg_partition_host(int64_t n, int kmax, const int32_t *nn, con
         stack.push_back(Seg{sg.b, mid, perm[(size_t)sg.b], idl});
     }
 }
+
+// The same bisection on GROUPS of `group` consecutive caller sites (group = 8: "octets"), so that an
+// internal site keeps its caller index modulo `group`:  internal = 8 * (position of its octet) + caller % 8.
+// Why: the kernels gather T_m[neighbour] from a tile staged in shared memory with 16-byte loads, eight
+// lanes (= eight consecutive sites) per wavefront; the eight loads are conflict-free when they fall into
+// eight different 16-byte bank groups, i.e. when the neighbours' slots differ modulo 8.  In a regularly
+// numbered lattice (the paper's row-major honeycomb cells) the k-th neighbours of eight consecutive
+// sites have eight different caller indices modulo 8, and an order that preserves the caller index
+// modulo 8 carries that over to the slots wherever the octets are placed; a site-by-site re-ordering
+// makes the residues random (2.3 wavefronts per gather instead of 1, profiles/r02a_tb2.md).
+// The trailing partial group, if any, stays last.  perm[new] = old.
+static inline void kg_partition_grouped(int64_t n, int kmax, const int32_t *nn, const int32_t *nl, int64_t leaf, int group,
+                                        std::vector<int32_t> &perm)
+{
+    if (group <= 1 || n < 2 * (int64_t)group) { kg_partition_host(n, kmax, nn, nl, leaf, perm); return; }
+    const int64_t ngf = n / group;                 // full groups (a trailing partial group is kept out)
+    // quotient graph: groups adjacent when any of their sites are
+    std::vector<int32_t> deg((size_t)ngf, 0), adj((size_t)ngf * group * kmax, -1);
+    const int64_t stride = (int64_t)group * kmax;
+    int kq = 0;
+    for (int64_t g = 0; g < ngf; ++g) {
+        int32_t *a = adj.data() + (size_t)g * stride;
+        int d = 0;
+        for (int64_t i = g * group; i < (g + 1) * group; ++i) {
+            int c = nn[i];
+            if (c > kmax) c = kmax;
+            for (int k = 0; k < c; ++k) {
+                const int32_t m = nl[(int64_t)k * n + i];
+                if (m < 0 || m >= n) continue;
+                const int32_t mg = (int32_t)(m / group);
+                if (mg == g || mg >= ngf) continue;
+                bool seen = false;
+                for (int q = 0; q < d; ++q) seen = seen || a[q] == mg;
+                if (!seen) a[d++] = mg;
+            }
+        }
+        deg[(size_t)g] = d;
+        kq = std::max(kq, d);
+    }
+    if (kq == 0) kq = 1;
+    std::vector<int32_t> nlq((size_t)ngf * kq, 0);
+    for (int64_t g = 0; g < ngf; ++g)
+        for (int k = 0; k < deg[(size_t)g]; ++k) nlq[(size_t)k * ngf + g] = adj[(size_t)g * stride + k];
+    adj.clear(); adj.shrink_to_fit();
+    std::vector<int32_t> pq;
+    kg_partition_host(ngf, kq, deg.data(), nlq.data(), std::max<int64_t>(1, leaf / group), pq);
+    perm.resize((size_t)n);
+    int64_t pos = 0;
+    for (int64_t g = 0; g < ngf; ++g)
+        for (int j = 0; j < group; ++j) perm[(size_t)pos++] = (int32_t)((int64_t)pq[(size_t)g] * group + j);
+    for (int64_t i = ngf * group; i < n; ++i) perm[(size_t)pos++] = (int32_t)i;
+}
