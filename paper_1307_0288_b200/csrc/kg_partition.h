@@ -96,7 +96,7 @@ static inline void kg_partition_host(int64_t n, int kmax, const int32_t *nn, con
 // numbered lattice (the paper's row-major honeycomb cells) the k-th neighbours of eight consecutive
 // sites have eight different caller indices modulo 8, and an order that preserves the caller index
 // modulo 8 carries that over to the slots wherever the octets are placed; a site-by-site re-ordering
-// makes the residues random (2.3 wavefronts per gather instead of 1, profiles/r02a_tb2.md).
+// makes the residues random (2.3 wavefronts per gather instead of 1, profiles/r02b_tb2.md).
 // The trailing partial group, if any, stays last.  perm[new] = old.
 static inline void kg_partition_grouped(int64_t n, int kmax, const int32_t *nn, const int32_t *nl, int64_t leaf, int group,
                                         std::vector<int32_t> &perm)

@@ -2,8 +2,9 @@
 // Alg. 5 (eq 38, eq 46) in their doubling forms (MODE_MOM2 / MODE_MOMX, see
 // kg_common.cuh), blocked in time inside the SM.
 //
-// Why: the one-step sweep (kg_staged.cuh) is bound by the bytes that cross L2 -> SM, not by DRAM
-// and not by latency (profiles/r02a_limits.md): T_m and T_{m-1} are read and T_{m+1} written for every
+// Why: the one-step sweep (kg_staged.cuh) sits on the DRAM line (profiles/r02b_tb2.md: 272 MB must move per
+// sweep of config 4 and it takes the time a copy of that size takes): T_m and T_{m-1} are read and T_{m+1}
+// written for every
 // step, 48 B + the matrix row per site-update.  Here a tile of CS consecutive sites — a compact patch
 // of the lattice after the re-ordering of kg_partition.h — is brought into shared memory together with
 // its two rings of halo sites
