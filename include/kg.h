@@ -270,7 +270,8 @@ enum {
                                 as in Alg. 6 / Alg. 7 */
     KG_OPT_REORDER = 12,     /* process-wide, read at create (kg_set_default_option): re-number the sites
                                 internally so that consecutive sites form compact patches of the lattice
-                                (recursive breadth-first bisection of the neighbour list; moments do not
+                                (recursive breadth-first bisection of the neighbour list, on groups of 8 consecutive
+                                caller sites so that a site keeps its caller index modulo 8; moments do not
                                 depend on the site order, vectors are permuted at the boundary of every call):
                                 1 always, 0 never, -1 (default) when n >= 65536 */
     KG_OPT_TWO_STEP = 13,    /* doubling moment loops on <= 2 contiguous columns run two Chebyshev steps per
