@@ -62,10 +62,17 @@ def site_updates(n: int, R: int, M: int, nt: int, n_p: int, doubling: bool = Fal
     """H~-applications one step really performs.  The oracle runs the literal
     Alg. 5 (M-1 applications per moment set); the CUDA path gets two moments per sweep from the
     product identity: M/2 applications per set when phi_L = phi_R (DOS, MSD),
-    2 * (M/2) for VAC, whose sweep advances both phi_L and phi_R; it is credited only with those."""
+    2 * (M/2) for VAC rows k >= 1, whose sweep advances both phi_L and phi_R (row k = 0 has phi_L = phi_R and
+    costs M/2); it is credited only with those."""
     per_set = M // 2 if doubling else M - 1
     dos = per_set
-    vac = 1 + (nt + 1) * (1 + (2 * (M // 2) if doubling else M - 1)) + nt * 2 * (n_p - 1)
+    # VAC: V phi once; per time point V psi_k + one moment set — at t = 0 phi_L = phi_R = V phi, so the
+    # doubling path runs it on one column (no velocity application either: chi_0 is copied), later rows
+    # advance both chains
+    if doubling:
+        vac = 1 + per_set + nt * (1 + 2 * per_set) + nt * 2 * (n_p - 1)
+    else:
+        vac = 1 + (nt + 1) * (1 + (M - 1)) + nt * 2 * (n_p - 1)
     # MSD row k = 0 is exactly 0 (psix_0 = 0) and is written, not computed: nt moment sets
     msd = nt * per_set + nt * 2 * (n_p - 1)
     per_vec = {"dos": dos, "vac": vac, "msd": msd}
@@ -303,26 +310,39 @@ def run_b200(args, cfg):
     mu0 = complex(mu_avg[0].item())
 
     # dominant kernel (about 60 % of the step, profiles/): the VAC moment sweep on the batch
-    # [V psi | chi] (C = 2R columns) with the two cross inner products per Chebyshev step.  On this
-    # config it is the TWO-STEP kernel kg_tb2_kernel<C, K, MODE_MOMX> (T_m+1 and T_m+2 per pass, tile + two
-    # halo rings in shared memory); kg_vac(M, n_steps = 0) is then velocity + column copy + first step +
-    # ceil((M/2 - 1)/2) passes + the final reduction, and the launch counter says which path ran.
-    mu_v0 = torch.empty((R, 1, M), dtype=torch.complex128, device="cuda")
-    B.vac(h, phi_dev, M, 0, cfg.dt_fs, mu=mu_v0)
+    # [V psi_k | chi_k] (C = 2R columns, rows k >= 1) with the two cross inner products per Chebyshev step.
+    # On this config it is the TWO-STEP kernel kg_tb2_kernel<C, K, MODE_MOMX> (T_m+1 and T_m+2 per pass, tile +
+    # two halo rings in shared memory).  One more time step of kg_vac = velocity + column copy + [first step +
+    # ceil((M/2 - 1)/2) passes + reduction] + one evolution of the 2R-column batch, so the moment loop is timed as
+    # kg_vac(n_steps = 2) - kg_vac(n_steps = 1) - kg_evolve(2R columns), all live CUDA events on the launching
+    # stream; the launch counter says which path ran.
     reps = 3
-    torch.cuda.synchronize()
-    l0 = h.launch_count
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    for _ in range(reps):
-        B.vac(h, phi_dev, M, 0, cfg.dt_fs, mu=mu_v0)
-    e1.record(stream)
-    torch.cuda.synchronize()
-    sweeps = (h.launch_count - l0) // reps - 4           # minus velocity, column copy, first step, reduction
+    C = 2 * R
+
+    def timed_calls(fn):
+        fn(); torch.cuda.synchronize()
+        l0 = h.launch_count
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(reps):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) * 1e3 / reps, (h.launch_count - l0) // reps
+
+    mu_v = [torch.empty((R, k + 1, M), dtype=torch.complex128, device="cuda") for k in (1, 2)]
+    phi_c = torch.from_numpy(W.random_phase_vectors(n, C, cfg.seed)).cuda()
+    evo_out = torch.empty_like(phi_c)
+    us_v1, l_v1 = timed_calls(lambda: B.vac(h, phi_dev, M, 1, cfg.dt_fs, mu=mu_v[0]))
+    us_v2, l_v2 = timed_calls(lambda: B.vac(h, phi_dev, M, 2, cfg.dt_fs, mu=mu_v[1]))
+    us_ev, l_ev = timed_calls(lambda: B.evolve(h, phi_c, -cfg.dt_fs, out=evo_out))
+    # (kg_evolve on caller-order vectors adds two row permutations to the 41 sweeps of the evolution inside
+    # kg_vac: 2 launches and 60 us in 85 ms, i.e. the pass time below is under-estimated by < 0.1 %)
+    sweeps = (l_v2 - l_v1) - (l_ev - 2) - 4              # minus velocity, column copy, first step, reduction
     steps = M // 2 - 1                                   # Chebyshev steps those launches perform
     two_step = sweeps < steps
-    kern_us = e0.elapsed_time(e1) * 1e3 / (reps * (sweeps + 1))     # the first step is a sweep of the same size
-    C = 2 * R
+    kern_us = (us_v2 - us_v1 - us_ev) / (sweeps + 1)     # the first step is a sweep of the same size
+    del mu_v, phi_c, evo_out
     peak, peak_src = peaks()
     ons = lat.onsite is not None
     if two_step:
@@ -360,6 +380,8 @@ def run_b200(args, cfg):
                                                   "fraction exceeds 1 — the roofline fraction is `frac`, on the bytes really required"},
                 "us_per_launch": kern_us,
                 "gsu_per_s": updates_launch / (kern_us * 1e-6) / 1e9, "traffic": ncu_traffic(tkey)}
+    if roofline["frac"] > 1.0:
+        roofline["warning"] = "frac > 1 against must-move bytes: the timed launches are not the kernel named here"
 
     # second kernel of the step (about 40 %): the DOS / MSD moment sweep on one column, kg_dos_moments(M) =
     # first step + passes + reduction, timed the same way

@@ -1374,7 +1374,14 @@ extern "C" int kg_vac(kg_hamiltonian *h, const kg_c128 *phi, int R, int M, int n
     const int64_t rstride = (int64_t)(n_steps + 1) * M;
     for (int k = 0; k <= n_steps; ++k) {
         // phi_L = V psi_k, phi_R = chi_k
-        if (h->doubling) {
+        if (h->doubling && k == 0) {
+            // t = 0: V psi_0 = V phi = chi_0, so phi_L = phi_R and the one-column doubling form applies
+            // (half the work of the cross form; C_m^VAC(0) = <V phi|T_m|V phi>)
+            c128 *X0 = (c128 *)pl;
+            if ((rc = copy_cols(h, S + R, R2, X0, R, R, st)) ||
+                (rc = moments_device(h, X0, R, X0, R, R, M, (c128 *)o.dev, rstride, st)))
+                return rc;
+        } else if (h->doubling) {
             // cross-doubling: [V psi_k | chi_k] advanced as one 2R-wide batch, two moments per sweep
             c128 *X0 = (c128 *)pl;
             if ((rc = velocity_device(h, S, R2, X0, R2, R, st)) || (rc = copy_cols(h, S + R, R2, X0 + R, R2, R, st)) ||

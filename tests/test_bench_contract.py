@@ -21,7 +21,7 @@ def test_site_update_accounting():
     assert lit["vac"] == (1 + 2 * (1 + M - 1) + 2 * (n_p - 1)) * per          # Alg. 2, two time points
     assert lit["msd"] == ((M - 1) + 2 * (n_p - 1)) * per                      # Alg. 3, pair recursion; row 0 = 0 is not computed
     assert dbl["dos"] == (M // 2) * per
-    assert dbl["vac"] == (1 + 2 * (1 + 2 * (M // 2)) + 2 * (n_p - 1)) * per   # both chains advanced
+    assert dbl["vac"] == (1 + M // 2 + (1 + 2 * (M // 2)) + 2 * (n_p - 1)) * per   # row 0: one column; row 1: both chains
     assert dbl["msd"] == ((M // 2) + 2 * (n_p - 1)) * per
     assert bench.mom_bytes_per_update(1) == 108.0 and bench.mom_bytes_per_update(8) == 69.5
     assert bench.mom_bytes_per_update(2, phi_l_stream=False) == 70.0
