@@ -282,7 +282,7 @@ enum {
                                 synchronisation per call) and the call returns KG_EINVAL; 0 (default): not checked —
                                 non-finite input gives non-finite output.  (The matrix is always checked at create.) */
     KG_OPT_ONE_LAUNCH = 15,  /* launch-bound sizes (all 512-element tiles of a batch fit the shared memory of one
-                                8-CTA cluster: n * R <= 16 K elements for the paper's model): the moment loop after
+                                8-CTA cluster: n * R <= 16 K elements for the paper's model; 9-16 tiles use a 16-CTA cluster when the device takes it): the moment loop after
                                 its first step runs as ONE kernel, one cluster barrier per Chebyshev step, vectors
                                 and matrix rows in distributed shared memory; bitwise equal to the per-step
                                 launches.  -1 (default) / 1: on when eligible, 0: off */

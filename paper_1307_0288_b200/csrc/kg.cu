@@ -123,6 +123,7 @@ struct kg_hamiltonian {
     int ndict;                // entries in use (0: hoppings do not fit a dictionary)
     int staged, stages, staged_ctas, alternate, doubling, clenshaw, pdl;   // options of the staged kernel
     int tb2;                  // KG_OPT_TWO_STEP: -1 auto, 0 off, 1 whenever a plan exists
+    int big_cluster;          // 1 until a 16-CTA cluster launch has been refused by the device
     int one_launch;           // KG_OPT_ONE_LAUNCH: -1 auto, 0 off: the moment loop of launch-bound sizes as one cluster kernel
     int check_input;          // KG_OPT_CHECK_INPUT: input vectors are scanned for NaN / Inf (one pass + a synchronisation)
     unsigned int *d_flag;     // device flag of that scan
@@ -588,7 +589,7 @@ static int create_from_device_list(kg_hamiltonian **out, int64_t n, int kmax, co
     h->s = s; h->e0 = e0; h->period = period;
     h->nl = h->nlp = nullptr; h->hop = h->xhop = h->onsite = nullptr;
     h->perm = h->iperm = nullptr;
-    h->tb2 = -1; memset(h->tbp, 0, sizeof(h->tbp));
+    h->tb2 = -1; memset(h->tbp, 0, sizeof(h->tbp)); h->big_cluster = 1;
     h->check_input = 0; h->d_flag = nullptr; h->one_launch = -1;
     h->ndict = 0; h->staged = 1; h->stages = 0; h->staged_ctas = 0; h->alternate = 1; h->doubling = 1; h->clenshaw = 1; h->pdl = -1;
     memset(h->dict, 0, sizeof(h->dict));
@@ -1023,11 +1024,22 @@ static int moments_device(kg_hamiltonian *h, const c128 *phiL, int ldL, const c1
             sa.nl = h->nl; sa.hop = h->hop; sa.onsite = h->onsite; sa.n = h->n; sa.ns = h->ns; sa.K = h->kmax;
             sa.ons = h->has_onsite ? 1 : 0;
             sa.t0 = phiR; sa.t1 = (const c128 *)ta; sa.phiL = phiL; sa.part = P; sa.m_end = m_end;
-            sa.ntiles = sp.ntiles; sa.vt = (sp.ntiles + SM_MAX_CLUSTER - 1) / SM_MAX_CLUSTER;
+            sa.ntiles = sp.ntiles;
             sa.alternate = h->alternate;
-            const int ncta = (sp.ntiles + sa.vt - 1) / sa.vt;
             h->launches++;
-            CUDA_TRY(kg_small_launch(mode, R, sa, ncta, (size_t)sa.vt * sm_tile_bytes(R, h->kmax, mode == MODE_MOM), h->device, st));
+            // 9-16 tiles: one tile per CTA in a 16-CTA cluster (non-portable size) when the device takes it,
+            // else two tiles per CTA in the portable 8-CTA cluster — same arithmetic, same partial slots
+            cudaError_t e = cudaErrorInvalidValue;
+            if (sp.ntiles > SM_MAX_CLUSTER && sp.ntiles <= SM_BIG_CLUSTER && h->big_cluster != 0) {
+                sa.vt = 1;
+                e = kg_small_launch(mode, R, sa, sp.ntiles, sm_tile_bytes(R, h->kmax, mode == MODE_MOM), h->device, st);
+                if (e != cudaSuccess) { (void)cudaGetLastError(); h->big_cluster = 0; }
+            }
+            if (e != cudaSuccess) {
+                sa.vt = (sp.ntiles + SM_MAX_CLUSTER - 1) / SM_MAX_CLUSTER;
+                const int ncta = (sp.ntiles + sa.vt - 1) / sa.vt;
+                CUDA_TRY(kg_small_launch(mode, R, sa, ncta, (size_t)sa.vt * sm_tile_bytes(R, h->kmax, mode == MODE_MOM), h->device, st));
+            }
         }
     } else if (want_graph(h, elems, st)) {
         cudaGraphExec_t exec = nullptr;

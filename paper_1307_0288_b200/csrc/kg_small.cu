@@ -25,6 +25,12 @@ cudaError_t launch_reg(const SmallArgs &a, int ncta, size_t smem, int device, cu
         if (e != cudaSuccess) return e;
         configured[dev] = smem;
     }
+    static bool big[64] = {false};
+    if (ncta > SM_MAX_CLUSTER && !big[dev]) {
+        cudaError_t e = cudaFuncSetAttribute(kg_small_reg_kernel<R, MODE, KU, VT>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        if (e != cudaSuccess) return e;
+        big[dev] = true;
+    }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)ncta);
     cfg.blockDim = dim3(SM_THREADS);
@@ -54,6 +60,12 @@ cudaError_t launch_ku(const SmallArgs &a, int ncta, size_t smem, int device, cud
         cudaError_t e = cudaFuncSetAttribute(kg_small_kernel<R, MODE, KU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         configured[dev] = smem;
+    }
+    static bool big[64] = {false};
+    if (ncta > SM_MAX_CLUSTER && !big[dev]) {
+        cudaError_t e = cudaFuncSetAttribute(kg_small_kernel<R, MODE, KU>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        if (e != cudaSuccess) return e;
+        big[dev] = true;
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)ncta);
@@ -87,7 +99,7 @@ cudaError_t launch_r(int mode, const SmallArgs &a, int ncta, size_t smem, int de
 
 cudaError_t kg_small_launch(int mode, int R, const SmallArgs &a, int ncta, size_t smem, int device, cudaStream_t st)
 {
-    if (ncta < 1 || ncta > SM_MAX_CLUSTER) return cudaErrorInvalidValue;
+    if (ncta < 1 || ncta > SM_BIG_CLUSTER) return cudaErrorInvalidValue;
     switch (R) {
     case 1: return launch_r<1>(mode, a, ncta, smem, device, st);
     case 2: return launch_r<2>(mode, a, ncta, smem, device, st);

@@ -18,7 +18,8 @@
 
 #define SM_TILE_E 512
 #define SM_THREADS 256
-#define SM_MAX_CLUSTER 8
+#define SM_MAX_CLUSTER 8        // portable cluster size
+#define SM_BIG_CLUSTER 16       // non-portable size B200 schedules inside one GPC (tried first for 9-16 tiles)
 
 struct SmallArgs {
     const int32_t *nl;       // [K][ns]
