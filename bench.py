@@ -345,64 +345,60 @@ def run_b200(args, cfg):
     del mu_v, phi_c, evo_out
     peak, peak_src = peaks()
     ons = lat.onsite is not None
-    if two_step:
-        # must-move bytes of a two-step pass, per site: T_m, T_m-1 read and T_m+1, T_m+2 written (64 B per
-        # column), 8 B of tile-local matrix row (4 x uint16), 8 B on-site energy; halo re-reads not counted
-        bytes_launch = (64.0 * C + 8.0 + (8.0 if ons else 0.0)) * n
-        kname = (f"kg_tb2_kernel<C={C}, K={lat.kmax}, MODE_MOMX, NSTEP=2> (two Chebyshev steps per pass on [phi_L | phi_R]: "
-                 "tile + two halo rings in shared memory, TMA-staged streams, four cross inner products per pass)")
-        bdef = ("must-move bytes of the launched two-step pass: (64 C + 8 + 8) B per site (T_m, T_m-1 read, T_m+1, T_m+2 written "
-                "for C columns; tile-local matrix row; on-site energy), no halo, no cache reuse between launches")
-        tkey = f"{cfg.name}_tb2_momx_C{C}"
-    else:
-        bytes_launch = must_move_bytes_per_update(C, lat.kmax, ons) * n * C
-        kname = (f"kg_staged_kernel<R={C}, MODE_MOMX> (fused T_m+1 = 2H~T_m - T_m-1 on [phi_L | phi_R] + the two cross inner "
-                 "products; TMA-staged streams, hopping dictionary, alternating sweep)")
-        bdef = ("must-move bytes of the launched one-step sweep: (48 + (4 K + 8)/C) B per site-update (T_m, T_m-1 read, T_m+1 "
-                "written, packed index + on-site row shared by the C columns)")
-        tkey = f"{cfg.name}_momx_R{C}"
-    if sweeps == 1 and steps > 2:
-        kname = "kg_small_kernel (launch-bound size: all Chebyshev steps after the first in ONE cluster launch, vectors in distributed shared memory)"
-    steps_per_launch = steps / sweeps if sweeps > 0 else 1.0
-    updates_launch = n * C * steps_per_launch
-    bytes_8d = mom_bytes_per_update(C, lat.kmax, phi_l_stream=False) * updates_launch
-    achieved = bytes_launch / (kern_us * 1e-6) / 1e9
-    roofline = {"bound": "hbm", "kernel": kname,
-                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0,
-                "bytes_per_launch": bytes_launch, "bytes_definition": bdef,
-                "chebyshev_steps_per_launch": steps_per_launch,
-                "survey_8d_general_ell": {"bytes_per_launch": bytes_8d, "achieved": bytes_8d / (kern_us * 1e-6) / 1e9,
-                                          "frac": bytes_8d / (kern_us * 1e-6) / 1e9 / peak,
-                                          "note": "SURVEY 8(d) doubling row, 48 + (12 K + 8)/C B per site-update of a one-step sweep "
-                                                  "with fp64 hoppings streamed, times the site-updates one launch performs; the launched "
-                                                  "kernel moves far fewer bytes (two steps per pass, hopping dictionary), so this "
-                                                  "fraction exceeds 1 — the roofline fraction is `frac`, on the bytes really required"},
-                "us_per_launch": kern_us,
-                "gsu_per_s": updates_launch / (kern_us * 1e-6) / 1e9, "traffic": ncu_traffic(tkey)}
-    if roofline["frac"] > 1.0:
-        roofline["warning"] = "frac > 1 against must-move bytes: the timed launches are not the kernel named here"
 
-    # second kernel of the step (about 40 %): the DOS / MSD moment sweep on one column, kg_dos_moments(M) =
-    # first step + passes + reduction, timed the same way
-    l0 = h.launch_count
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    for _ in range(reps):
-        B.dos_moments(h, phi_dev, M, mu=mu_dos)
-    e1.record(stream)
-    torch.cuda.synchronize()
-    sweeps1 = (h.launch_count - l0) // reps - 2                 # minus first step, reduction
-    us1 = e0.elapsed_time(e1) * 1e3 / (reps * (sweeps1 + 1))
-    spl1 = steps / sweeps1 if sweeps1 > 0 else 1.0
-    bytes1 = ((64.0 * R + 8.0 + (8.0 if ons else 0.0)) * n) if sweeps1 < steps else must_move_bytes_per_update(R, lat.kmax, ons) * n * R
-    roofline["second_kernel"] = {
-        "kernel": ("kg_small_kernel" if (sweeps1 == 1 and steps > 2) else f"kg_tb2_kernel<C={R}, K={lat.kmax}, MODE_MOM2, NSTEP=2>" if sweeps1 < steps else f"kg_staged_kernel<R={R}, MODE_MOM2>") +
-                  " (DOS / MSD moment sweeps, phi_L = phi_R)",
-        "us_per_launch": us1, "chebyshev_steps_per_launch": spl1, "bytes_per_launch": bytes1,
-        "achieved": bytes1 / (us1 * 1e-6) / 1e9, "frac": bytes1 / (us1 * 1e-6) / 1e9 / peak,
-        "gsu_per_s": n * R * spl1 / (us1 * 1e-6) / 1e9,
-        "traffic": ncu_traffic(f"{cfg.name}_tb2_mom2_C{R}" if sweeps1 < steps else f"{cfg.name}_mom2_R{R}")}
+    def kernel_block(mode, cols, us, nsweeps):
+        """roofline entry of one moment kernel: `nsweeps` launches perform `steps` Chebyshev steps on `cols` columns"""
+        two = nsweeps < steps
+        if nsweeps == 1 and steps > 2:
+            kname = "kg_small_kernel (launch-bound size: all Chebyshev steps after the first in ONE cluster launch, vectors in distributed shared memory)"
+        elif two:
+            kname = (f"kg_tb2_kernel<C={cols}, K={lat.kmax}, {mode}, NSTEP=2> (two Chebyshev steps per pass: tile + two halo rings in "
+                     "shared memory, TMA-staged streams, four inner products per pass)")
+        else:
+            kname = (f"kg_staged_kernel<R={cols}, {mode}> (fused T_m+1 = 2H~T_m - T_m-1 + two inner products; TMA-staged streams, "
+                     "hopping dictionary, alternating sweep)")
+        if two:
+            # must-move bytes of a two-step pass, per site: T_m, T_m-1 read and T_m+1, T_m+2 written (64 B per
+            # column), 8 B of tile-local matrix row (4 x uint16), 8 B on-site energy; halo re-reads not counted
+            bl = (64.0 * cols + 8.0 + (8.0 if ons else 0.0)) * n
+            bdef = ("must-move bytes of the launched two-step pass: (64 C + 8 + 8) B per site (T_m, T_m-1 read, T_m+1, T_m+2 written "
+                    "for C columns; tile-local matrix row; on-site energy), no halo, no cache reuse between launches")
+            tkey = f"{cfg.name}_tb2_{'momx' if mode == 'MODE_MOMX' else 'mom2'}_C{cols}"
+        else:
+            bl = must_move_bytes_per_update(cols, lat.kmax, ons) * n * cols
+            bdef = ("must-move bytes of the launched one-step sweep: (48 + (4 K + 8)/C) B per site-update (T_m, T_m-1 read, T_m+1 "
+                    "written, packed index + on-site row shared by the C columns)")
+            tkey = f"{cfg.name}_{'momx' if mode == 'MODE_MOMX' else 'mom2'}_R{cols}"
+        spl = steps / nsweeps if nsweeps > 0 else 1.0
+        upd = n * cols * spl
+        b8d = mom_bytes_per_update(cols, lat.kmax, phi_l_stream=False) * upd
+        ach = bl / (us * 1e-6) / 1e9
+        blk = {"bound": "hbm", "kernel": kname, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+               "peak_source": peak_src, "frac_of_nominal_8TBs": ach / 8000.0, "bytes_per_launch": bl, "bytes_definition": bdef,
+               "chebyshev_steps_per_launch": spl,
+               "survey_8d_general_ell": {"bytes_per_launch": b8d, "achieved": b8d / (us * 1e-6) / 1e9, "frac": b8d / (us * 1e-6) / 1e9 / peak,
+                                         "note": "SURVEY 8(d) doubling row, 48 + (12 K + 8)/C B per site-update of a one-step sweep "
+                                                 "with fp64 hoppings streamed, times the site-updates one launch performs; the launched "
+                                                 "kernel moves far fewer bytes (two steps per pass, hopping dictionary), so this "
+                                                 "fraction exceeds 1 - the roofline fraction is `frac`, on the bytes really required"},
+               "us_per_launch": us, "gsu_per_s": upd / (us * 1e-6) / 1e9, "traffic": ncu_traffic(tkey)}
+        if blk["frac"] > 1.0:
+            blk["warning"] = "frac > 1 against must-move bytes: the timed launches are not the kernel named here"
+        return blk
+
+    momx = kernel_block("MODE_MOMX", C, kern_us, sweeps)
+    # the DOS / MSD / VAC-row-0 moment sweep on R columns: kg_dos_moments(M) = first step + passes + reduction
+    us_d, l_d = timed_calls(lambda: B.dos_moments(h, phi_dev, M, mu=mu_dos))
+    sweeps1 = l_d - 2                                           # minus first step, reduction
+    mom2 = kernel_block("MODE_MOM2", R, us_d / (sweeps1 + 1), sweeps1)
+    # which of the two dominates the step: launches per bench step x time per launch
+    t_momx = nt * (sweeps + 1) * momx["us_per_launch"]                  # VAC rows k = 1 .. nt
+    t_mom2 = (2 + nt) * (sweeps1 + 1) * mom2["us_per_launch"]           # DOS, VAC row 0, MSD rows 1 .. nt
+    step_us = ms / args.steps * 1e3
+    momx["share_of_step"] = t_momx / step_us
+    mom2["share_of_step"] = t_mom2 / step_us
+    roofline, other = (mom2, momx) if t_mom2 >= t_momx else (momx, mom2)
+    roofline["second_kernel"] = other
 
     if rank != 0:
         ctx.finalize()
