@@ -17,7 +17,7 @@ SRC = [os.path.join(CSRC, f) for f in ("kg.cu", "kg_staged_k2.cu", "kg_staged_k3
                                        "kg_staged_k6.cu", "kg_staged_k9.cu", "kg_tb2.cu", "kg_small.cu")]
 HEADERS = [os.path.join(CSRC, f) for f in ("kg_common.cuh", "kg_kernels.cuh", "kg_staged.cuh",
                                            "kg_staged_impl.cuh", "kg_staged_launch.h", "kg_partition.h",
-                                           "kg_tb2.cuh", "kg_tb2_launch.h", "kg_small.cuh", "kg_small_launch.h")]
+                                           "kg_tb2.cuh", "kg_tb2_launch.h", "kg_small.cuh", "kg_small_launch.h", "kg_smem_config.h")]
 DEPS = SRC + HEADERS + [os.path.join(ROOT, "include", "kg.h")]
 LIB = os.path.join(HERE, "libkg.so")
 OBJ_DIR = os.path.join(HERE, "build")

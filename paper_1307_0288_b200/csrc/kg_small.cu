@@ -1,6 +1,7 @@
 // Single-launch moment loop for launch-bound sizes (kg_small.cuh): template dispatch and cluster launch.
 #include "kg_small.cuh"
 #include "kg_small_launch.h"
+#include "kg_smem_config.h"
 
 namespace {
 
@@ -18,19 +19,8 @@ cudaError_t launch_t(const SmallArgs &a, int ncta, size_t smem, int device, cuda
 template <int R, int MODE, int KU, int VT>
 cudaError_t launch_reg(const SmallArgs &a, int ncta, size_t smem, int device, cudaStream_t st)
 {
-    static size_t configured[64] = {0};
-    const int dev = device & 63;
-    if (configured[dev] < smem) {
-        cudaError_t e = cudaFuncSetAttribute(kg_small_reg_kernel<R, MODE, KU, VT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured[dev] = smem;
-    }
-    static bool big[64] = {false};
-    if (ncta > SM_MAX_CLUSTER && !big[dev]) {
-        cudaError_t e = cudaFuncSetAttribute(kg_small_reg_kernel<R, MODE, KU, VT>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-        if (e != cudaSuccess) return e;
-        big[dev] = true;
-    }
+    static KgSmemConfig cfg_once;
+    if (cudaError_t e = cfg_once.ensure(kg_small_reg_kernel<R, MODE, KU, VT>, device, smem, ncta > SM_MAX_CLUSTER)) return e;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)ncta);
     cfg.blockDim = dim3(SM_THREADS);
@@ -54,19 +44,8 @@ cudaError_t launch_ku(const SmallArgs &a, int ncta, size_t smem, int device, cud
         if (a.vt == 1) return launch_reg<R, MODE, KU, 1>(a, ncta, smem, device, st);
         if (a.vt == 2) return launch_reg<R, MODE, KU, 2>(a, ncta, smem, device, st);
     }
-    static size_t configured[64] = {0};
-    const int dev = device & 63;
-    if (configured[dev] < smem) {
-        cudaError_t e = cudaFuncSetAttribute(kg_small_kernel<R, MODE, KU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured[dev] = smem;
-    }
-    static bool big[64] = {false};
-    if (ncta > SM_MAX_CLUSTER && !big[dev]) {
-        cudaError_t e = cudaFuncSetAttribute(kg_small_kernel<R, MODE, KU>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-        if (e != cudaSuccess) return e;
-        big[dev] = true;
-    }
+    static KgSmemConfig cfg_once;
+    if (cudaError_t e = cfg_once.ensure(kg_small_kernel<R, MODE, KU>, device, smem, ncta > SM_MAX_CLUSTER)) return e;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)ncta);
     cfg.blockDim = dim3(SM_THREADS);

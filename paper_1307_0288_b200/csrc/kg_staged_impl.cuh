@@ -2,6 +2,7 @@
 // width KG_STAGED_K, included by kg_staged_k<K>.cu.  Each such file is its own translation unit.
 #include "kg_staged.cuh"
 #include "kg_staged_launch.h"
+#include "kg_smem_config.h"
 
 #ifndef KG_STAGED_K
 #error "define KG_STAGED_K before including kg_staged_impl.cuh"
@@ -12,14 +13,8 @@ namespace {
 template <int R, int K, int MODE, bool ONS, bool DICT>
 cudaError_t launch_t(const StagedArgs &a, const StagedLaunch &l, cudaStream_t st)
 {
-    static size_t configured[64] = {0};
-    const int dev = l.device & 63;
-    if (configured[dev] < l.smem) {
-        cudaError_t e = cudaFuncSetAttribute(kg_staged_kernel<R, K, MODE, ONS, DICT>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)l.smem);
-        if (e != cudaSuccess) return e;
-        configured[dev] = l.smem;
-    }
+    static KgSmemConfig cfg_once;
+    if (cudaError_t e = cfg_once.ensure(kg_staged_kernel<R, K, MODE, ONS, DICT>, l.device, l.smem)) return e;
     if (!l.pdl) {
         kg_staged_kernel<R, K, MODE, ONS, DICT><<<l.grid, SG_THREADS, l.smem, st>>>(a);
         return cudaGetLastError();

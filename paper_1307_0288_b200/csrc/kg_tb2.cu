@@ -1,20 +1,15 @@
 // Two-step Chebyshev kernels (kg_tb2.cuh): template dispatch (K, columns, mode, ONS, steps per pass).
 #include "kg_tb2.cuh"
 #include "kg_tb2_launch.h"
+#include "kg_smem_config.h"
 
 namespace {
 
 template <int C, int K, int MODE, bool ONS, int NSTEP>
 cudaError_t launch_t(const Tb2Args &a, int grid, size_t smem, int device, cudaStream_t st)
 {
-    static size_t configured[64] = {0};
-    const int dev = device & 63;
-    if (configured[dev] < smem) {
-        cudaError_t e = cudaFuncSetAttribute(kg_tb2_kernel<C, K, MODE, ONS, NSTEP>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured[dev] = smem;
-    }
+    static KgSmemConfig cfg_once;
+    if (cudaError_t e = cfg_once.ensure(kg_tb2_kernel<C, K, MODE, ONS, NSTEP>, device, smem)) return e;
     kg_tb2_kernel<C, K, MODE, ONS, NSTEP><<<grid, TB_THREADS, smem, st>>>(a);
     return cudaGetLastError();
 }
