@@ -46,3 +46,23 @@ def test_bench_line_on_small_config():
     assert b["e2e"]["h2d_bytes_per_step"] > 0 and b["e2e"]["d2h_bytes_per_step"] > 0
     r = b["roofline"]
     assert r["bound"] == "hbm" and r["unit"] == "GB/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
+
+
+def test_reference_arm_line_on_the_cpu():
+    """`bench.py --impl reference` (the oracle timed on the host cores) prints ONE JSON line with the driver's keys,
+    the oracle described in cpu_baseline, and an e2e block repeating the value; no GPU involved."""
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--shrink", "25",
+                          "--steps", "2", "--warmup", "1"], capture_output=True, text=True, cwd=ROOT, timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [ln for ln in out.stdout.splitlines() if ln.strip()]
+    assert len(lines) == 1
+    b = json.loads(lines[0])
+    assert b["impl"] == "reference" and b["steps"] == 2 and b["warmup"] == 1 and b["higher_is_better"] is True
+    for key in ("metric", "value", "unit", "n_gpus", "ms_per_step", "scaling", "vs_baseline", "dtype", "data", "config",
+                "cpu_baseline", "e2e", "gpu_launches"):
+        assert key in b, key
+    assert b["value"] > 0 and b["gpu_launches"] == 0 and b["vs_baseline"] is None
+    cb = b["cpu_baseline"]
+    assert cb["kind"] == "oracle" and cb["cores"] == 1 and cb["value"] == b["value"] and "recursion + dot" in cb["sample"]
+    assert cb["cpu_model"] and cb["host_cores_available"] >= 1
+    assert b["e2e"] == {"value": b["value"], "unit": b["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
