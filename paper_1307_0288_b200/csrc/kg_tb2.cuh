@@ -98,6 +98,19 @@ __device__ __forceinline__ void tb_cp_async_arrive(uint32_t bar)
     asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
 }
 
+// T_{m+1} / T_{m+2} go out with an L2 evict_last hint: they are what the next pass (which sweeps the tiles
+// in the opposite direction) reads first, the streams read by this pass are dead (one-column pass: -2 %)
+__device__ __forceinline__ uint64_t tb_keep_policy()
+{
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void tb_store_keep(c128 *p, c128 v, uint64_t pol)
+{
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+
 // one matrix row from shared memory: KP packed uint16 as KP/2 words
 template <int KP>
 __device__ __forceinline__ void tb_load_row(const uint16_t *rows_s, int row, uint32_t (&w)[KP / 2])
@@ -140,6 +153,7 @@ __global__ void __launch_bounds__(TB_THREADS, 1) kg_tb2_kernel(const Tb2Args a)
     const size_t off_rows = off_hid + (size_t)(cap1 + cap2) * 4;
 
     const int tid = threadIdx.x;
+    const uint64_t keep = tb_keep_policy();
     const uint32_t fa0 = sg_smem_u32(bars), fb0 = sg_smem_u32(bars + TB_MAX_STAGES), em0 = sg_smem_u32(bars + 2 * TB_MAX_STAGES),
                    fh0 = sg_smem_u32(bars + 3 * TB_MAX_STAGES);
     if (tid == 0) {
@@ -274,7 +288,7 @@ __global__ void __launch_bounds__(TB_THREADS, 1) kg_tb2_kernel(const Tb2Args a)
 #pragma unroll
                         for (int c = 0; c < C; ++c) {
                             if (NSTEP == 2) Tp[(size_t)row * C + (c ^ sw)] = t1[q][c];
-                            a.next1[(site0 + row) * C + (c ^ sw)] = t1[q][c];
+                            tb_store_keep(a.next1 + (site0 + row) * C + (c ^ sw), t1[q][c], keep);
                         }
                         if (MODE == MODE_MOM2) {
                             // (C = 2: register slot c holds column c ^ sw; the per-column sums are un-swizzled at the end)
@@ -335,7 +349,7 @@ __global__ void __launch_bounds__(TB_THREADS, 1) kg_tb2_kernel(const Tb2Args a)
                     }
                     if (row < nown) {
 #pragma unroll
-                        for (int c = 0; c < C; ++c) a.next2[(site0 + row) * C + (c ^ sw)] = t2[c];
+                        for (int c = 0; c < C; ++c) tb_store_keep(a.next2 + (site0 + row) * C + (c ^ sw), t2[c], keep);
                         if (MODE == MODE_MOM2) {
 #pragma unroll
                             for (int c = 0; c < C; ++c) {
