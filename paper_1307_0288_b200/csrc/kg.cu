@@ -90,6 +90,7 @@ enum {
     WS_RAW0, WS_RAW1,                      // caller-order staging between a host pointer and the permutation kernel
     WS_TC, WS_TD,                          // third / fourth Chebyshev vector of the two-step kernel
     WS_MU,                                 // device moments when the caller's mu is host memory
+    WS_PLANE,                              // one column pair [n][2] of a wider batch (two-step kernel on R > 2)
     WS_COUNT
 };
 
@@ -943,6 +944,8 @@ static bool want_graph(const kg_hamiltonian *h, int64_t elems, cudaStream_t st)
     return elems <= (int64_t)1 << 21;      // auto: launch-bound sizes only
 }
 
+static int copy_cols(kg_hamiltonian *h, const c128 *src, int ld_src, c128 *dst, int ld_dst, int ncols, cudaStream_t st);
+
 // mu[r*mu_rstride + m] = <phiL_r | T_m(H~) | phiR_r>, m < M
 // cross = true: phiL == phiR is the batch [phi_L | phi_R] with R columns in total (MODE_MOMX);
 // mu gets R/2 rows.
@@ -955,6 +958,35 @@ static int moments_device(kg_hamiltonian *h, const c128 *phiL, int ldL, const c1
     const int PR = cross ? R / 2 : R;                        // columns of a partial row / rows of mu
     const StagedPlan sp = staged_plan(h, mode, R);
     int rc;
+    // wider doubling batches on a lattice the two-step kernel serves: column pair by column pair.  The kernel
+    // keeps a matrix row and its columns in per-thread registers, which stops at two columns; a pair is
+    // copied into a [n][2] plane (1 of ~M/4 passes) and run on its own — the matrix is re-read per pair
+    // (16 of 144 B per site and pass) against 32 instead of 48 B of vector traffic per site-update.
+    if (dbl && R > 2 && ldL == R && ldR == R && M / 2 >= 3) {
+        Tb2Launch t2;
+        if ((rc = tb2_plan(h, mode, 2, st, &t2))) return rc;
+        if (t2.ok) {
+            void *pl;
+            if ((rc = ws_get(h, WS_PLANE, (size_t)h->n * 2 * 16, &pl))) return rc;
+            c128 *P2 = (c128 *)pl;
+            if (cross) {
+                // batch [phi_L (R/2 columns) | phi_R (R/2 columns)]: plane r = [phi_L,r | phi_R,r]
+                const int Rh = R / 2;
+                for (int r = 0; r < Rh; ++r) {
+                    if ((rc = copy_cols(h, phiR + r, R, P2, 2, 1, st)) || (rc = copy_cols(h, phiR + Rh + r, R, P2 + 1, 2, 1, st)) ||
+                        (rc = moments_device(h, P2, 2, P2, 2, 2, M, mu + (int64_t)r * mu_rstride, mu_rstride, st, true)))
+                        return rc;
+                }
+            } else {
+                for (int r = 0; r < R; r += 2) {
+                    if ((rc = copy_cols(h, phiR + r, R, P2, 2, 2, st)) ||
+                        (rc = moments_device(h, P2, 2, P2, 2, 2, M, mu + (int64_t)r * mu_rstride, mu_rstride, st)))
+                        return rc;
+                }
+            }
+            return KG_OK;
+        }
+    }
     // two Chebyshev steps per pass (kg_tb2.cuh) when the vectors are contiguous [n][R], R <= 2
     Tb2Launch tl;
     tl.ok = false;

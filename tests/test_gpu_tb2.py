@@ -191,3 +191,31 @@ def test_reordering_is_a_permutation_and_keeps_results(B, reordered):
     assert host(B.apply_velocity(h1, phi)).tobytes() == host(B.apply_velocity(h0, phi)).tobytes()
     assert relerr(host(B.dos_moments(h1, phi, 40)), host(B.dos_moments(h0, phi, 40))) <= 1e-13
     assert relerr(host(B.evolve(h1, phi, 1.3)), host(B.evolve(h0, phi, 1.3))) <= 1e-14
+
+
+@pytest.mark.parametrize("R", [4, 8])
+def test_two_step_wider_batches_pair_by_pair(B, kgo, reordered, R):
+    """R = 4, 8: the doubling moment loops run the two-column two-step kernel on one column pair after the other
+    (DOS and MSD: pairs (0,1), (2,3), ...; VAC: the pair [V psi_r | chi_r] of every vector); every vector against the
+    oracle, and the launch count shows that no one-step sweep ran."""
+    lat, s = sheet(True)
+    olat = to_oracle_lattice(kgo, lat)
+    h = B.from_lattice(lat, lat.x, lat.period_x, 0.0, s)
+    h.set_option(B.KG_OPT_TWO_STEP, 1)
+    M, nt, dt = 21, 2, 0.6
+    phi = W.random_phase_vectors(lat.n, R, 5)
+    B.dos_moments(h, dev(phi), M)                      # builds the per-tile plan
+    l0 = h.launch_count
+    dos = host(B.dos_moments(h, dev(phi), M))
+    passes = (M // 2 - 1 + 1) // 2
+    assert h.launch_count - l0 == 1 + (R // 2) * (1 + 1 + passes + 1)      # permutation + per pair: copy, first step, passes, reduction
+    vac = host(B.vac(h, dev(phi), M, nt, dt))
+    msd = host(B.msd(h, dev(phi), M, nt, dt))
+    for r in range(R):
+        v = phi[:, r].copy()
+        assert relerr(dos[r], kgo.dos_moments(olat, 0.0, s, v, M)) <= TOL
+        assert relerr(vac[r], kgo.vac(olat, olat.x, olat.period_x, 0.0, s, v, M, nt, dt)) <= TOL
+        assert relerr(msd[r], kgo.msd(olat, olat.x, olat.period_x, 0.0, s, v, M, nt, dt)) <= TOL
+    h.set_option(B.KG_OPT_TWO_STEP, 0)
+    assert relerr(host(B.dos_moments(h, dev(phi), M)), dos) <= 1e-12
+    assert relerr(host(B.vac(h, dev(phi), M, nt, dt)), vac) <= 1e-12
