@@ -274,8 +274,9 @@ enum {
                                 caller sites so that a site keeps its caller index modulo 8; moments do not
                                 depend on the site order, vectors are permuted at the boundary of every call):
                                 1 always, 0 never, -1 (default) when n >= 65536 */
-    KG_OPT_TWO_STEP = 13,    /* doubling moment loops on <= 2 contiguous columns run two Chebyshev steps per
-                                pass with the tile + two halo rings in shared memory (temporal blocking):
+    KG_OPT_TWO_STEP = 13,    /* doubling moment loops run two Chebyshev steps per pass with the tile + two halo
+                                rings in shared memory (temporal blocking), on <= 2 contiguous columns at a time
+                                (wider batches one column pair after the other):
                                 1 whenever the plan fits, 0 never, -1 (default) when the sites are re-ordered
                                 and there are at least four 1024-element tiles per SM */
     KG_OPT_CHECK_INPUT = 14, /* 1: every input vector is scanned for NaN / Inf (one extra pass and a stream
