@@ -276,7 +276,7 @@ enum {
                                 1 always, 0 never, -1 (default) when n >= 65536 */
     KG_OPT_TWO_STEP = 13,    /* doubling moment loops run two Chebyshev steps per pass with the tile + two halo
                                 rings in shared memory (temporal blocking), on <= 2 contiguous columns at a time
-                                (wider batches one column pair after the other):
+                                (wider batches as column-pair planes side by side in one launch, when the batch exceeds the L2):
                                 1 whenever the plan fits, 0 never, -1 (default) when the sites are re-ordered
                                 and there are at least four 1024-element tiles per SM */
     KG_OPT_CHECK_INPUT = 14, /* 1: every input vector is scanned for NaN / Inf (one extra pass and a stream

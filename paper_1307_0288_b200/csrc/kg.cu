@@ -132,7 +132,7 @@ struct kg_hamiltonian {
     void *ws[WS_COUNT];
     size_t ws_bytes[WS_COUNT];
     size_t matrix_bytes;
-    int device, num_sms;
+    int device, num_sms, l2_bytes;
     int threads, blocks_per_sm, use_graphs;
     int64_t launches;
     std::vector<GraphEntry> graphs;
@@ -468,14 +468,19 @@ static int tb2_build_plan(kg_hamiltonian *h, int C, cudaStream_t st)
 struct Tb2Launch { bool ok; int grid, nst; size_t smem; };
 
 // Is the two-step kernel to be used for a doubling moment loop on C contiguous columns?
-static int tb2_plan(kg_hamiltonian *h, int mode, int C, cudaStream_t st, Tb2Launch *out)
+static int tb2_plan(kg_hamiltonian *h, int mode, int C, int nplanes, cudaStream_t st, Tb2Launch *out)
 {
     out->ok = false;
     if (h->tb2 == 0 || !h->staged || !h->doubling || C > 2 || (mode == MODE_MOMX && C != 2) ||
         (mode != MODE_MOM2 && mode != MODE_MOMX))
         return KG_OK;
     const int64_t nt = (h->n + tb_cs(C) - 1) / tb_cs(C);
-    if (h->tb2 < 0 && (!h->perm || nt < 4 * (int64_t)h->num_sms)) return KG_OK;    // auto: re-ordered sites, >= 4 tiles per SM
+    if (h->tb2 < 0 && (!h->perm || nt * nplanes < 4 * (int64_t)h->num_sms)) return KG_OK;    // auto: re-ordered sites, >= 4 tiles per SM
+    // auto, wider batches as column-pair planes: only when three vectors of the batch do not fit L2 — an
+    // L2-resident wide batch is served faster by the one-step kernel, which shares a matrix row among all
+    // R columns (config 2: 13.8 us per one-step sweep of 8 columns against 35 us per two-step pass)
+    if (h->tb2 < 0 && nplanes > 1 && (int64_t)h->n * C * nplanes * 48 <= (int64_t)h->l2_bytes) return KG_OK;
+    if (nplanes > h->num_sms) return KG_OK;
     Tb2Plan &tp = h->tbp[C - 1];
     if (!tp.built) { int rc = tb2_build_plan(h, C, st); if (rc) return rc; }
     if (!tp.ok) return KG_OK;
@@ -485,7 +490,7 @@ static int tb2_plan(kg_hamiltonian *h, int mode, int C, cudaStream_t st, Tb2Laun
     if (out->nst > TB_MAX_STAGES) out->nst = TB_MAX_STAGES;
     if (out->nst < 2) return KG_OK;
     out->smem = TB_HEADER + (size_t)out->nst * stage;
-    out->grid = (int)std::min<int64_t>(tp.ntiles, (int64_t)h->num_sms);
+    out->grid = (int)std::min<int64_t>(tp.ntiles, (int64_t)h->num_sms / nplanes);     // CTAs per plane
     out->ok = true;
     return KG_OK;
 }
@@ -498,6 +503,7 @@ static Tb2Args tb2_base_args(const kg_hamiltonian *h, int C)
     a.tinfo = tp.tinfo; a.rows = tp.rows; a.hid = tp.hid; a.hons = tp.hons; a.onsite = h->onsite;
     memcpy(a.dict, h->dict, sizeof(a.dict));
     a.n = h->n; a.cap1 = tp.cap1; a.cap2 = tp.cap2; a.ntiles = tp.ntiles;
+    a.nplanes = 1; a.plane_stride = 0;
     return a;
 }
 
@@ -603,7 +609,8 @@ static int create_from_device_list(kg_hamiltonian **out, int64_t n, int kmax, co
     auto cleanup = [&](int code) { if (d_flags) cudaFree(d_flags); kg_destroy_hamiltonian(h); return code; };
     cudaError_t e;
     if ((e = cudaGetDevice(&h->device)) != cudaSuccess ||
-        (e = cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, h->device)) != cudaSuccess)
+        (e = cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, h->device)) != cudaSuccess ||
+        (e = cudaDeviceGetAttribute(&h->l2_bytes, cudaDevAttrL2CacheSize, h->device)) != cudaSuccess)
         return cleanup(fail(KG_ECUDA, "device query: %s", cudaGetErrorString(e)));
     const size_t slab = (size_t)h->ns * kmax;
     h->matrix_bytes = slab * (4 + 8 + 8) + (size_t)h->ns * 8;
@@ -958,39 +965,17 @@ static int moments_device(kg_hamiltonian *h, const c128 *phiL, int ldL, const c1
     const int PR = cross ? R / 2 : R;                        // columns of a partial row / rows of mu
     const StagedPlan sp = staged_plan(h, mode, R);
     int rc;
-    // wider doubling batches on a lattice the two-step kernel serves: column pair by column pair.  The kernel
-    // keeps a matrix row and its columns in per-thread registers, which stops at two columns; a pair is
-    // copied into a [n][2] plane (1 of ~M/4 passes) and run on its own — the matrix is re-read per pair
-    // (16 of 144 B per site and pass) against 32 instead of 48 B of vector traffic per site-update.
-    if (dbl && R > 2 && ldL == R && ldR == R && M / 2 >= 3) {
-        Tb2Launch t2;
-        if ((rc = tb2_plan(h, mode, 2, st, &t2))) return rc;
-        if (t2.ok) {
-            void *pl;
-            if ((rc = ws_get(h, WS_PLANE, (size_t)h->n * 2 * 16, &pl))) return rc;
-            c128 *P2 = (c128 *)pl;
-            if (cross) {
-                // batch [phi_L (R/2 columns) | phi_R (R/2 columns)]: plane r = [phi_L,r | phi_R,r]
-                const int Rh = R / 2;
-                for (int r = 0; r < Rh; ++r) {
-                    if ((rc = copy_cols(h, phiR + r, R, P2, 2, 1, st)) || (rc = copy_cols(h, phiR + Rh + r, R, P2 + 1, 2, 1, st)) ||
-                        (rc = moments_device(h, P2, 2, P2, 2, 2, M, mu + (int64_t)r * mu_rstride, mu_rstride, st, true)))
-                        return rc;
-                }
-            } else {
-                for (int r = 0; r < R; r += 2) {
-                    if ((rc = copy_cols(h, phiR + r, R, P2, 2, 2, st)) ||
-                        (rc = moments_device(h, P2, 2, P2, 2, 2, M, mu + (int64_t)r * mu_rstride, mu_rstride, st)))
-                        return rc;
-                }
-            }
-            return KG_OK;
-        }
-    }
-    // two Chebyshev steps per pass (kg_tb2.cuh) when the vectors are contiguous [n][R], R <= 2
+    // two Chebyshev steps per pass (kg_tb2.cuh) when the vectors are contiguous [n][R].  The kernel keeps a
+    // matrix row and its columns in per-thread registers, which stops at two columns: a wider batch is split
+    // into column-pair PLANES [n][2] — (2p, 2p+1) for phi_L = phi_R, (phi_L,r, phi_R,r) for the cross form — that
+    // ONE launch per pass serves side by side, each plane on its share of the CTAs.
     Tb2Launch tl;
     tl.ok = false;
-    if (dbl && ldL == R && ldR == R && M / 2 >= 3 && (rc = tb2_plan(h, mode, R, st, &tl))) return rc;
+    const int CP = R <= 2 ? R : 2;                                  // columns per plane
+    const int nplanes = R / CP;
+    if (dbl && ldL == R && ldR == R && M / 2 >= 3 && (R <= 2 || R % 2 == 0) &&
+        (rc = tb2_plan(h, mode, CP, nplanes, st, &tl)))
+        return rc;
     const int grid = tl.ok ? tl.grid : sp.ok ? sp.grid : grid_for(h, elems);   // one partial row shape for all kernels of the call
     void *ta, *tb, *part;
     if ((rc = ws_get(h, WS_TA, (size_t)elems * 16, &ta)) || (rc = ws_get(h, WS_TB, (size_t)elems * 16, &tb)) ||
@@ -999,19 +984,41 @@ static int moments_device(kg_hamiltonian *h, const c128 *phiL, int ldL, const c1
     if (tl.ok) {
         void *tc, *td;
         if ((rc = ws_get(h, WS_TC, (size_t)elems * 16, &tc)) || (rc = ws_get(h, WS_TD, (size_t)elems * 16, &td))) return rc;
-        const size_t prow = (size_t)grid * PR;
+        const size_t prow = (size_t)grid * PR;                      // partial rows [grid = CTAs per plane][PR], plane-major columns
         c128 *P = (c128 *)part;
-        // m = 1: T_1 = H~ T_0 and the partials of moments 0, 1, 2 (one-thread-per-element kernel)
+        // m = 1: T_1 = H~ T_0 and the partials of moments 0, 1, 2 (one-thread-per-element kernel, whole batch)
         StepArgs a = base_args(h);
         a.phiL = phiL; a.ld_L = ldL; a.alpha = 1.0;
         a.cur = phiR; a.ld_cur = ldR; a.next = (c128 *)ta;
         a.partial0 = P; a.partial = P + prow; a.partial2 = P + 2 * prow;
         CUDA_TRY(launch_step(h, mode, true, R, a, grid, st));
         // steps m = 2 .. M/2 in pairs; step m makes T_m and the partials of moments 2m - 1 and 2m
-        Tb2Args ta2 = tb2_base_args(h, R);
+        Tb2Args ta2 = tb2_base_args(h, CP);
         ta2.nstages = tl.nst;
+        ta2.nplanes = nplanes; ta2.plane_stride = nplanes > 1 ? h->n * CP : 0;
         const c128 *prev = phiR, *cur = (const c128 *)ta;
         std::vector<c128 *> freeb = {(c128 *)tb, (c128 *)tc, (c128 *)td};
+        if (nplanes > 1) {
+            // T_0 and T_1 from [n][R] into planes [nplanes][n][2]
+            void *p0;
+            if ((rc = ws_get(h, WS_PLANE, (size_t)elems * 16, &p0))) return rc;
+            c128 *P0 = (c128 *)p0, *P1 = (c128 *)tb;
+            const int Rh = R / 2;
+            for (int p = 0; p < nplanes; ++p) {
+                c128 *d0 = P0 + (size_t)p * h->n * 2, *d1 = P1 + (size_t)p * h->n * 2;
+                if (cross) {
+                    if ((rc = copy_cols(h, phiR + p, R, d0, 2, 1, st)) || (rc = copy_cols(h, phiR + Rh + p, R, d0 + 1, 2, 1, st)) ||
+                        (rc = copy_cols(h, (const c128 *)ta + p, R, d1, 2, 1, st)) ||
+                        (rc = copy_cols(h, (const c128 *)ta + Rh + p, R, d1 + 1, 2, 1, st)))
+                        return rc;
+                } else if ((rc = copy_cols(h, phiR + 2 * p, R, d0, 2, 2, st)) || (rc = copy_cols(h, (const c128 *)ta + 2 * p, R, d1, 2, 2, st))) {
+                    return rc;
+                }
+            }
+            prev = P0; cur = P1;
+            freeb = {(c128 *)ta, (c128 *)tc, (c128 *)td};
+        }
+        const c128 *keep_in = nplanes > 1 ? nullptr : phiR;          // the caller's phi_R is never written
         const int m_end = M / 2 + 1;
         int pass = 0;
         for (int m = 2; m < m_end; ++pass) {
@@ -1022,18 +1029,18 @@ static int moments_device(kg_hamiltonian *h, const c128 *phiL, int ldL, const c1
             ta2.p3 = P + (size_t)(2 * m + 1) * prow; ta2.p4 = P + (size_t)(2 * m + 2) * prow;
             ta2.reverse = h->alternate ? (pass & 1) : 0;
             h->launches++;
-            CUDA_TRY(kg_tb2_launch(h->kmax, mode, R, h->has_onsite, nstep, ta2, grid, tl.smem, h->device, st));
-            // rotate: the two oldest vectors become free (the caller's phiR is never written)
+            CUDA_TRY(kg_tb2_launch(h->kmax, mode, CP, h->has_onsite, nstep, ta2, grid * nplanes, tl.smem, h->device, st));
+            // rotate: the two oldest vectors become free
             c128 *old_prev = const_cast<c128 *>(prev), *old_cur = const_cast<c128 *>(cur);
             if (nstep == 2) {
                 prev = freeb[0]; cur = freeb[1];
                 freeb.erase(freeb.begin(), freeb.begin() + 2);
-                if (old_prev != phiR) freeb.push_back(old_prev);
+                if (old_prev != keep_in) freeb.push_back(old_prev);
                 freeb.push_back(old_cur);
             } else {
                 prev = cur; cur = freeb[0];
                 freeb.erase(freeb.begin());
-                if (old_prev != phiR) freeb.push_back(old_prev);
+                if (old_prev != keep_in) freeb.push_back(old_prev);
             }
             m += nstep;
         }

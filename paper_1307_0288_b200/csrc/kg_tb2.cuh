@@ -60,6 +60,8 @@ struct Tb2Args {
     double dict[16];
     int64_t n;
     int cap1, cap2, ntiles, reverse, nstages;
+    int nplanes;             // independent [n][C] batches served by one launch (CTAs are split evenly among them)
+    int64_t plane_stride;    // elements between consecutive planes in cur / prev / next1 / next2
     const c128 *cur, *prev;  // T_m, T_{m-1}   [n][C]
     c128 *next1, *next2;     // T_{m+1}, T_{m+2}
     c128 *p1, *p2, *p3, *p4; // moment partials [grid][PR] of moments 2m+1 .. 2m+4 (p3, p4: NSTEP = 2)
@@ -167,12 +169,17 @@ __global__ void __launch_bounds__(TB_THREADS, 1) kg_tb2_kernel(const Tb2Args a)
     }
     __syncthreads();
 
-    const int my_tiles = ((int)blockIdx.x < a.ntiles) ? (a.ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
+    // planes: gridDim.x = nplanes * cpp; CTA (plane, bl) sweeps the tiles bl, bl + cpp, ... of its plane
+    const int cpp = (int)gridDim.x / a.nplanes, plane = (int)blockIdx.x / cpp, bl = (int)blockIdx.x - plane * cpp;
+    const c128 *const cur_p = a.cur + plane * a.plane_stride, *const prev_p = a.prev + plane * a.plane_stride;
+    c128 *const next1_p = a.next1 + plane * a.plane_stride;
+    c128 *const next2_p = NSTEP == 2 ? a.next2 + plane * a.plane_stride : nullptr;
+    const int my_tiles = (bl < a.ntiles) ? (a.ntiles - 1 - bl) / cpp + 1 : 0;
     c128 s1[PR], s2[PR], s3[PR], s4[PR];
 #pragma unroll
     for (int c = 0; c < PR; ++c) s1[c] = s2[c] = s3[c] = s4[c] = make_double2(0.0, 0.0);
 
-    auto tile_of = [&](int j) { int t = (int)blockIdx.x + j * (int)gridDim.x; return a.reverse ? a.ntiles - 1 - t : t; };
+    auto tile_of = [&](int j) { int t = bl + j * cpp; return a.reverse ? a.ntiles - 1 - t : t; };
 
     if (tid == TB_CONSUMERS) {
         // ---------------- warp 8, one lane: TMA bulk copies of everything contiguous ----------------
@@ -206,8 +213,8 @@ __global__ void __launch_bounds__(TB_THREADS, 1) kg_tb2_kernel(const Tb2Args a)
                 sg_mbar_arrive(fh);
             }
             sg_mbar_expect_tx(fa, 2u * vb + rb + ob + gb);
-            sg_bulk_g2s(sb, a.cur + site0 * C, vb, fa);
-            sg_bulk_g2s(sb + (uint32_t)off_tp, a.prev + site0 * C, vb, fa);
+            sg_bulk_g2s(sb, cur_p + site0 * C, vb, fa);
+            sg_bulk_g2s(sb + (uint32_t)off_tp, prev_p + site0 * C, vb, fa);
             sg_bulk_g2s(sb + (uint32_t)off_rows, a.rows + (size_t)t * (CS + cap1) * KP, rb, fa);
             if (ONS) sg_bulk_g2s(sb + (uint32_t)off_ons, a.onsite + site0, ob, fa);
             if (gb) sg_bulk_g2s(sb + (uint32_t)off_hons, a.hons + (size_t)t * cap1, gb, fa);
@@ -227,8 +234,8 @@ __global__ void __launch_bounds__(TB_THREADS, 1) kg_tb2_kernel(const Tb2Args a)
                 const int64_t g = (int64_t)hid_s[q] * C;
 #pragma unroll
                 for (int c = 0; c < C; ++c) {
-                    tb_cp_async16(tm_s + (uint32_t)((CS + q) * C + c) * 16u, a.cur + g + c);
-                    if (NSTEP == 2 && q < n1) tb_cp_async16(tp_s + (uint32_t)((CS + q) * C + c) * 16u, a.prev + g + c);
+                    tb_cp_async16(tm_s + (uint32_t)((CS + q) * C + c) * 16u, cur_p + g + c);
+                    if (NSTEP == 2 && q < n1) tb_cp_async16(tp_s + (uint32_t)((CS + q) * C + c) * 16u, prev_p + g + c);
                 }
             }
             tb_cp_async_arrive(fb0 + 8 * s);
@@ -288,7 +295,7 @@ __global__ void __launch_bounds__(TB_THREADS, 1) kg_tb2_kernel(const Tb2Args a)
 #pragma unroll
                         for (int c = 0; c < C; ++c) {
                             if (NSTEP == 2) Tp[(size_t)row * C + (c ^ sw)] = t1[q][c];
-                            tb_store_keep(a.next1 + (site0 + row) * C + (c ^ sw), t1[q][c], keep);
+                            tb_store_keep(next1_p + (site0 + row) * C + (c ^ sw), t1[q][c], keep);
                         }
                         if (MODE == MODE_MOM2) {
                             // (C = 2: register slot c holds column c ^ sw; the per-column sums are un-swizzled at the end)
@@ -349,7 +356,7 @@ __global__ void __launch_bounds__(TB_THREADS, 1) kg_tb2_kernel(const Tb2Args a)
                     }
                     if (row < nown) {
 #pragma unroll
-                        for (int c = 0; c < C; ++c) tb_store_keep(a.next2 + (site0 + row) * C + (c ^ sw), t2[c], keep);
+                        for (int c = 0; c < C; ++c) tb_store_keep(next2_p + (site0 + row) * C + (c ^ sw), t2[c], keep);
                         if (MODE == MODE_MOM2) {
 #pragma unroll
                             for (int c = 0; c < C; ++c) {
@@ -378,7 +385,7 @@ __global__ void __launch_bounds__(TB_THREADS, 1) kg_tb2_kernel(const Tb2Args a)
     }
 #pragma unroll
     for (int c = 0; c < PR; ++c) {
-        const int64_t slot = (int64_t)blockIdx.x * PR + c;
+        const int64_t slot = ((int64_t)bl * a.nplanes + plane) * PR + c;      // [cpp][nplanes * PR]: plane-major columns
         c128 tot = tb_block_sum(s1[c], red);
         if (tid == 0) a.p1[slot] = tot;
         tot = tb_block_sum(s2[c], red);

@@ -194,10 +194,10 @@ def test_reordering_is_a_permutation_and_keeps_results(B, reordered):
 
 
 @pytest.mark.parametrize("R", [4, 8])
-def test_two_step_wider_batches_pair_by_pair(B, kgo, reordered, R):
-    """R = 4, 8: the doubling moment loops run the two-column two-step kernel on one column pair after the other
-    (DOS and MSD: pairs (0,1), (2,3), ...; VAC: the pair [V psi_r | chi_r] of every vector); every vector against the
-    oracle, and the launch count shows that no one-step sweep ran."""
+def test_two_step_wider_batches_as_column_pair_planes(B, kgo, reordered, R):
+    """R = 4, 8: the doubling moment loops run the two-column two-step kernel on column-pair planes, all planes in
+    one launch per pass (DOS and MSD: pairs (0,1), (2,3), ...; VAC: the pair [V psi_r | chi_r] of every vector);
+    every vector against the oracle, and the launch count shows that no one-step sweep ran."""
     lat, s = sheet(True)
     olat = to_oracle_lattice(kgo, lat)
     h = B.from_lattice(lat, lat.x, lat.period_x, 0.0, s)
@@ -208,7 +208,7 @@ def test_two_step_wider_batches_pair_by_pair(B, kgo, reordered, R):
     l0 = h.launch_count
     dos = host(B.dos_moments(h, dev(phi), M))
     passes = (M // 2 - 1 + 1) // 2
-    assert h.launch_count - l0 == 1 + (R // 2) * (1 + 1 + passes + 1)      # permutation + per pair: copy, first step, passes, reduction
+    assert h.launch_count - l0 == 1 + 1 + R + passes + 1      # permutation, first step, T_0 / T_1 into R/2 planes, passes, reduction
     vac = host(B.vac(h, dev(phi), M, nt, dt))
     msd = host(B.msd(h, dev(phi), M, nt, dt))
     for r in range(R):
