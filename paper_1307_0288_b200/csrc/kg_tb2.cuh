@@ -28,6 +28,11 @@
 // paper's model eq 13) and C = 1 or 2 columns per site.  NSTEP = 1 is the same kernel doing a
 // single step (odd step counts), so that one call uses one grid and one shape of moment partials.
 //
+// Wider batches: a launch can serve `nplanes` independent [n][C] batches (column pairs of an [n][R] batch,
+// kg.cu: moments_device) side by side — gridDim.x = nplanes * cpp, CTA (plane, bl) sweeps the tiles bl,
+// bl + cpp, ... of its plane with the SAME per-tile plan, and writes its partial into the plane's columns of
+// the common row [cpp][nplanes * PR], which is the layout of the first-step kernel and of kg_reduce_partials.
+//
 // Determinism: tile -> CTA -> thread -> row assignment is a pure function of the launch shape, sums run
 // in a fixed order, the block tree is fixed, kg_reduce_partials adds the CTA partials in CTA order.
 #pragma once
