@@ -206,6 +206,42 @@ int kg_kpm_reconstruct(const kg_c128 *mu, int64_t rows, int M, int jackson, doub
                        void *stream);
 
 /*
+ * kg_kpm_reconstruct_noalloc — the same reconstruction (eqs 29-31, Jackson damping eq 35
+ * P:190-192; same formula, same kernels, same results as kg_kpm_reconstruct) for callers that are
+ * not in a position to allocate device memory: a program that has already given all of the GPU's
+ * memory to an arena of its own (a framework's caching allocator; a run whose Chebyshev vectors
+ * were sized to fill the card), where one more cudaMalloc or a growing memory pool fails, and a
+ * program that post-processes moments inside a loop with a latency budget that a fresh allocation
+ * (which can stall the whole device) would break.  This call allocates nothing — no cudaMalloc,
+ * cudaMallocAsync, cudaFree or allocating library routine, on the host or on the device.  The
+ * damped weights (2 - delta_m0) g_m, the one temporary the reconstruction needs, are written to
+ * a fixed array inside the library image instead:
+ *
+ *   LIMIT    M <= KG_KPM_NOALLOC_MAX_M (16384 weights = 128 KiB of device memory, occupied on
+ *            every GPU that loads libkg until the process exits).  A longer series is KG_EINVAL
+ *            with the limit in kg_last_error(); use kg_kpm_reconstruct for it.
+ *   POINTERS mu [rows][M], energies_eV [n_energies] and f [rows][n_energies] must all be DEVICE
+ *            memory (a host array would have to be staged, which takes an allocation): a host
+ *            pointer is KG_EINVAL.  The energy grid is therefore never checked on the host;
+ *            entries with |(E_j - E0)/s| >= 1 give NaN in f, as for a device grid in
+ *            kg_kpm_reconstruct.
+ *   SHARING  there is ONE weight array per GPU, used by every call from every thread and stream.
+ *            A call rewrites entries 0..M-1 before it reads them and reads no others, so what an
+ *            earlier call left behind does no harm; but two calls whose kernels can overlap on
+ *            the GPU (issued on different streams without an ordering between them) race on the
+ *            array and give wrong results.  Issue them on one stream, or order them with events.
+ *   FIRST CALL  the first call on each device looks the array's device address up
+ *            (cudaGetSymbolAddress, with the calling thread's current device) and keeps it; make
+ *            that first call outside any stream capture.  Later calls only enqueue two kernels
+ *            on `stream`.  Device ordinals >= 64 are KG_EUNSUPPORTED.
+ * Does not synchronise.  Other arguments as kg_kpm_reconstruct.
+ */
+#define KG_KPM_NOALLOC_MAX_M 16384
+int kg_kpm_reconstruct_noalloc(const kg_c128 *mu, int64_t rows, int M, int jackson, double e0_eV,
+                               double scale_eV, const double *energies_eV, int n_energies,
+                               double *f, void *stream);
+
+/*
  * kg_transport — running conductivities and ballistic length / conductance on a (t_k, E_j) grid,
  * t_k = k dt, k = 0..n_steps, from reconstructed functions (kg_kpm_reconstruct):
  *   rho[j] = rho~(E_j);  fvac[k][j] = rho~ C_vv(E_j,t_k);  fmsd[k][j] = rho~ DeltaX^2(E_j,t_k).

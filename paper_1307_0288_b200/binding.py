@@ -60,6 +60,8 @@ _lib.kg_transport.argtypes = [_int, _int, _dbl, _dbl, _dbl] + [_vp] * 9
 _lib.kg_fourier_moments.argtypes = [_vp, _vp, _vp, _int, _int, _dbl, _dbl, _vp, _vp]
 _lib.kg_ftm_reconstruct.argtypes = [_vp, _i64, _int, _int, _dbl, _vp, _int, _vp, _vp]
 _lib.kg_kpm_reconstruct.argtypes = [_vp, _i64, _int, _int, _dbl, _dbl, _vp, _int, _vp, _vp]
+_lib.kg_kpm_reconstruct_noalloc.argtypes = [_vp, _i64, _int, _int, _dbl, _dbl, _vp, _int, _vp, _vp]
+KG_KPM_NOALLOC_MAX_M = 16384
 
 
 class KgError(RuntimeError):
@@ -251,6 +253,23 @@ def kpm_reconstruct(mu, e0_eV, scale_eV, energies_eV, jackson=True, stream=None)
         f = torch.empty(lead + (ne,), dtype=torch.float64, device=mu.device)
     _check(_lib.kg_kpm_reconstruct(_ptr(mu), rows, M, int(bool(jackson)), float(e0_eV), float(scale_eV),
                                    _ptr(energies_eV), ne, _ptr(f), _stream(stream)))
+    return f
+
+
+def kpm_reconstruct_noalloc(mu, e0_eV, scale_eV, energies_eV, f, jackson=True, stream=None):
+    """kg_kpm_reconstruct_noalloc: the reconstruction of ``kpm_reconstruct`` for callers that cannot
+    allocate GPU memory (all of it already belongs to their own arena, or an allocation would stall
+    a latency-bound loop).  Nothing is allocated here either: ``mu`` [..., M], ``energies_eV`` and the
+    output ``f`` [..., n_energies] are CUDA tensors the caller made beforehand, M must not exceed
+    ``KG_KPM_NOALLOC_MAX_M``, and the weights go to one fixed array per GPU inside libkg — so calls
+    that could overlap on the GPU (different streams) must be ordered by the caller.  Returns ``f``."""
+    M = int(mu.shape[-1])
+    lead = tuple(mu.shape[:-1])
+    rows = int(np.prod(lead)) if lead else 1
+    ne = int(energies_eV.shape[0])
+    assert tuple(f.shape) == lead + (ne,) and f.dtype in (torch.float64, np.float64)
+    _check(_lib.kg_kpm_reconstruct_noalloc(_ptr(mu), rows, M, int(bool(jackson)), float(e0_eV), float(scale_eV),
+                                           _ptr(energies_eV), ne, _ptr(f), _stream(stream)))
     return f
 
 

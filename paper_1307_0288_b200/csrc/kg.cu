@@ -16,6 +16,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1648,6 +1649,85 @@ extern "C" int kg_ftm_reconstruct(const kg_c128 *F, int64_t rows, int Nm, int wi
                                                     (const double *)d_en, n_energies, (double *)d_f);
     CUDA_TRY(cudaGetLastError());
     if (!f_dev) CUDA_TRY(cudaMemcpyAsync(f, d_f, (size_t)rows * n_energies * 8, cudaMemcpyDeviceToHost, st));
+    return KG_OK;
+    });
+}
+
+// --------------------------------------------------------------------------------------
+// kg_kpm_reconstruct_noalloc — the KPM reconstruction for callers that must not allocate.
+//
+// kg_kpm_reconstruct keeps the damped weights (2 - delta_m0) g_m in a temporary device buffer
+// taken from the stream-ordered pool.  Some users of this library cannot afford that: a host
+// application that has handed every byte of HBM to its own arena (a framework's caching
+// allocator, or a job whose Chebyshev vectors were sized to fill the 180 GB) gets an
+// out-of-memory error from any further cudaMalloc / pool growth, and a service that reconstructs
+// spectra inside a latency-bound loop cannot take the device-wide stall a fresh allocation may
+// cost.  For them the weights live in the fixed array below, which is part of the library image:
+// KG_KPM_NOALLOC_MAX_M doubles = 128 KiB on every GPU that loads libkg, held until the process
+// exits.  The call path underneath issues two kernel launches and nothing else — no cudaMalloc,
+// cudaMallocAsync, cudaFree, no copy, no std::vector.
+//
+// The array is ONE per device, shared by every call and every stream: a call overwrites entries
+// 0..M-1 (entries beyond M keep whatever an earlier call left and are never read, so nothing has
+// to be cleared first), and two calls that overlap on the GPU — different streams, or different
+// host threads — race on it.
+//
+// In host code `g_kpm_noalloc_w` is only a stand-in for the symbol; the device address is fetched
+// with cudaGetSymbolAddress once per device (with that device current) the first time the entry
+// point is called there, and cached.  That first call loads the module's data on the device, so
+// it should be made outside any stream capture.
+// --------------------------------------------------------------------------------------
+static __device__ __align__(256) double g_kpm_noalloc_w[KG_KPM_NOALLOC_MAX_M];
+
+#define KG_NOALLOC_MAX_DEVICES 64
+static std::mutex g_noalloc_lock;
+static double *g_noalloc_w_dev[KG_NOALLOC_MAX_DEVICES];   // device address of the array, per device ordinal
+
+static int noalloc_weights(double **w)
+{
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= KG_NOALLOC_MAX_DEVICES)
+        return fail(KG_EUNSUPPORTED, "kg_kpm_reconstruct_noalloc: device ordinal %d is beyond the %d this entry point tracks",
+                    dev, KG_NOALLOC_MAX_DEVICES);
+    std::lock_guard<std::mutex> hold(g_noalloc_lock);
+    if (!g_noalloc_w_dev[dev]) {
+        void *p = nullptr;
+        CUDA_TRY(cudaGetSymbolAddress(&p, g_kpm_noalloc_w));
+        if (!p) return fail(KG_ECUDA, "kg_kpm_reconstruct_noalloc: cudaGetSymbolAddress returned a null address");
+        g_noalloc_w_dev[dev] = (double *)p;
+    }
+    *w = g_noalloc_w_dev[dev];
+    return KG_OK;
+}
+
+extern "C" int kg_kpm_reconstruct_noalloc(const kg_c128 *mu, int64_t rows, int M, int jackson, double e0_eV,
+                                          double scale_eV, const double *energies_eV, int n_energies,
+                                          double *f, void *stream)
+{
+    return guarded([&]() -> int {
+    if (!mu || !energies_eV || !f) return fail(KG_EINVAL, "kg_kpm_reconstruct_noalloc: NULL argument");
+    if (rows <= 0 || rows > 65535 || M < 1 || n_energies < 1)
+        return fail(KG_EINVAL, "kg_kpm_reconstruct_noalloc: need 1 <= rows <= 65535, M >= 1, n_energies >= 1");
+    if (M > KG_KPM_NOALLOC_MAX_M)
+        return fail(KG_EINVAL, "kg_kpm_reconstruct_noalloc: M = %d exceeds the fixed weight table of "
+                    "KG_KPM_NOALLOC_MAX_M = %d entries; use kg_kpm_reconstruct (which allocates) for longer series",
+                    M, KG_KPM_NOALLOC_MAX_M);
+    if (!(scale_eV > 0.0) || !std::isfinite(scale_eV) || !std::isfinite(e0_eV))
+        return fail(KG_EINVAL, "kg_kpm_reconstruct_noalloc: scale must be positive and finite");
+    // a host array would have to be staged in device memory, i.e. allocated: not here
+    if (!is_device_ptr(mu) || !is_device_ptr(energies_eV) || !is_device_ptr(f))
+        return fail(KG_EINVAL, "kg_kpm_reconstruct_noalloc: mu, energies_eV and f must be device memory "
+                    "(staging a host array needs an allocation; kg_kpm_reconstruct does that)");
+    double *d_w = nullptr;
+    int rc;
+    if ((rc = noalloc_weights(&d_w))) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    kg_kpm_weights<<<(M + 255) / 256, 256, 0, st>>>(M, jackson, d_w);
+    dim3 grid((n_energies + 127) / 128, (unsigned)rows);
+    kg_kpm_reconstruct_kernel<<<grid, 128, 0, st>>>((const c128 *)mu, rows, M, d_w, e0_eV, scale_eV, energies_eV,
+                                                    n_energies, f);
+    CUDA_TRY(cudaGetLastError());
     return KG_OK;
     });
 }
