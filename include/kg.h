@@ -198,8 +198,11 @@ int kg_bessel_terms(double x, double bessel_eps, int *np_out, double *j, int cap
  *   energies_eV [n_energies], host or device; every |x_j| must be < 1: a host grid is checked
  *             (KG_EINVAL), a device grid is not read back — such entries of f are NaN
  *   f         [rows][n_energies] fp64, host or device
- * Runs as CUDA kernels on `stream`; temporaries are stream-ordered pool allocations
- * (cudaMallocAsync), so the call neither allocates with cudaMalloc nor synchronises.
+ * Runs as CUDA kernels on `stream`; temporaries are stream-ordered allocations from a memory pool
+ * that the library creates per device at the first post-processing call there (kg_kpm_reconstruct,
+ * kg_transport, kg_ftm_reconstruct) and keeps, with whatever it has grown to, until the process
+ * exits; the application's default pool is not touched.  Once the pool is warm the call neither
+ * allocates with cudaMalloc nor synchronises.
  */
 int kg_kpm_reconstruct(const kg_c128 *mu, int64_t rows, int M, int jackson, double e0_eV,
                        double scale_eV, const double *energies_eV, int n_energies, double *f,
@@ -309,7 +312,16 @@ enum {
                                 (recursive breadth-first bisection of the neighbour list, on groups of 8 consecutive
                                 caller sites so that a site keeps its caller index modulo 8; moments do not
                                 depend on the site order, vectors are permuted at the boundary of every call):
-                                1 always, 0 never, -1 (default) when n >= 65536 */
+                                1 always, 0 never, -1 (default) when n >= 65536.
+                                COST: only the moment loops (kg_moments, kg_dos_moments, kg_vac, kg_msd) gain from the
+                                new order.  On a re-ordered handle every call that takes or returns a vector pays one
+                                extra pass over it per vector argument (a gather into internal order on the way in, a
+                                scatter on the way out) and keeps staging buffers of n * R * 16 bytes each in the
+                                workspace: kg_apply_velocity is 3 sweeps instead of 1, each kg_evolve of a caller-driven
+                                loop 2 extra sweeps, kg_evolve_x 4.  A handle used mainly for kg_evolve /
+                                kg_apply_velocity is better created with the option at 0.  Moments are bitwise
+                                reproducible for a given setting, not across settings (the summation order follows
+                                the site order) */
     KG_OPT_TWO_STEP = 13,    /* doubling moment loops run two Chebyshev steps per pass with the tile + two halo
                                 rings in shared memory (temporal blocking), on <= 2 contiguous columns at a time
                                 (wider batches as column-pair planes side by side in one launch, when the batch exceeds the L2):

@@ -447,11 +447,16 @@ static int tb2_build_plan(kg_hamiltonian *h, int C, cudaStream_t st)
         for (int64_t i = s0; i < s1; ++i) fill((int)(i - s0), i);
         for (int j = 0; j < n1; ++j) fill(CS + j, hl[(size_t)j]);
     }
-    cudaError_t e;
-    if ((e = cudaMalloc(&tp.tinfo, (size_t)ntiles * sizeof(int2))) != cudaSuccess ||
-        (e = cudaMalloc(&tp.rows, rows.size() * 2)) != cudaSuccess || (e = cudaMalloc(&tp.hid, hid.size() * 4)) != cudaSuccess ||
-        (e = cudaMalloc(&tp.hons, (size_t)ntiles * cap1 * 8)) != cudaSuccess)
-        return fail(KG_ENOMEM, "two-step plan allocation: %s", cudaGetErrorString(e));
+    if (cudaMalloc(&tp.tinfo, (size_t)ntiles * sizeof(int2)) != cudaSuccess ||
+        cudaMalloc(&tp.rows, rows.size() * 2) != cudaSuccess || cudaMalloc(&tp.hid, hid.size() * 4) != cudaSuccess ||
+        cudaMalloc(&tp.hons, (size_t)ntiles * cap1 * 8) != cudaSuccess) {
+        // no room for the plan: not an error of the call — release the part that was allocated and leave
+        // tp.ok = false, the one-step kernels serve the handle
+        cudaGetLastError();
+        cudaFree(tp.tinfo); cudaFree(tp.rows); cudaFree(tp.hid); cudaFree(tp.hons);
+        tp.tinfo = nullptr; tp.rows = nullptr; tp.hid = nullptr; tp.hons = nullptr;
+        return KG_OK;
+    }
     tp.bytes = (size_t)ntiles * sizeof(int2) + rows.size() * 2 + hid.size() * 4 + (size_t)ntiles * cap1 * 8;
     CUDA_TRY(cudaMemcpyAsync(tp.tinfo, tinfo.data(), (size_t)ntiles * sizeof(int2), cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemcpyAsync(tp.rows, rows.data(), rows.size() * 2, cudaMemcpyHostToDevice, st));
@@ -623,7 +628,7 @@ static int create_from_device_list(kg_hamiltonian **out, int64_t n, int kmax, co
         return cleanup(fail(KG_ECUDA, "memset: %s", cudaGetErrorString(e)));
     // site re-ordering: recursive breadth-first bisection of the neighbour list on the host
     // (kg_partition.h), so that every aligned block of consecutive internal sites is a compact patch
-    if (g_reorder > 0 || (g_reorder < 0 && n >= KG_REORDER_MIN_SITES)) {
+    if (g_reorder > 0 || (g_reorder < 0 && n >= KG_REORDER_MIN_SITES)) try {
         std::vector<int32_t> h_nn((size_t)n), h_nl((size_t)n * kmax), perm, iperm((size_t)n);
         if ((e = cudaMemcpyAsync(h_nn.data(), d_nn, (size_t)n * 4, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
             (e = cudaMemcpyAsync(h_nl.data(), d_nl, (size_t)n * kmax * 4, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
@@ -638,6 +643,8 @@ static int create_from_device_list(kg_hamiltonian **out, int64_t n, int kmax, co
             (e = cudaMemcpyAsync(h->iperm, iperm.data(), (size_t)n * 4, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
             (e = cudaStreamSynchronize(st)) != cudaSuccess)          // the host vectors go out of scope
             return cleanup(fail(KG_ECUDA, "permutation upload: %s", cudaGetErrorString(e)));
+    } catch (const std::bad_alloc &) {       // the host tables of the bisection: release the half-built handle
+        return cleanup(fail(KG_ENOMEM, "host allocation failed in the site re-ordering"));
     }
     const int grid = (int)std::min<int64_t>((h->ns + 255) / 256, (int64_t)h->num_sms * 8);
     kg_build_matrix<<<grid, 256, 0, st>>>(n, h->ns, kmax, d_nn, d_nl, d_hop, d_ons, d_x, period, e0, s,
@@ -682,12 +689,13 @@ static int create_from_device_list(kg_hamiltonian **out, int64_t n, int kmax, co
             (e = cudaStreamSynchronize(st)) != cudaSuccess)
             return cleanup2(fail(KG_ECUDA, "kg_dict_collect: %s", cudaGetErrorString(e)));
         if ((unsigned int)tab[15] == 0) {
-            std::vector<double> vals;
+            double vals[15];
+            int nvals = 0;
             for (int q = 0; q < 15; ++q)
-                if (tab[q] != SG_DICT_EMPTY) { double v; memcpy(&v, &tab[q], 8); vals.push_back(v); }
-            std::sort(vals.begin(), vals.end());
-            h->ndict = 1 + (int)vals.size();
-            for (size_t q = 0; q < vals.size(); ++q) h->dict[1 + q] = vals[q];
+                if (tab[q] != SG_DICT_EMPTY) memcpy(&vals[nvals++], &tab[q], 8);
+            std::sort(vals, vals + nvals);
+            h->ndict = 1 + nvals;
+            for (int q = 0; q < nvals; ++q) h->dict[1 + q] = vals[q];
             if ((e = cudaMemcpyAsync(d_dict, h->dict, 16 * 8, cudaMemcpyHostToDevice, st)) != cudaSuccess)
                 return cleanup2(fail(KG_ECUDA, "dictionary: %s", cudaGetErrorString(e)));
             kg_dict_pack<<<grid, 256, 0, st>>>(h->nl, h->hop, (int64_t)slab, d_dict, h->ndict, h->nlp);
@@ -735,29 +743,43 @@ struct TmpDev {
     }
 };
 
-// Stream-ordered temporaries of the handle-free post-processing calls: cudaMallocAsync from the
-// device's default pool (kept warm: release threshold = never), cudaFreeAsync when the call
-// returns — no cudaMalloc, no cudaFree and no synchronisation once the pool has grown.
+// Stream-ordered temporaries of the handle-free post-processing calls: cudaMallocFromPoolAsync from a
+// memory pool the library owns (one per device, created at the first such call there, kept warm:
+// release threshold = never, alive until the process exits), cudaFreeAsync when the call returns — no
+// cudaMalloc, no cudaFree and no synchronisation once the pool has grown.  The application's default
+// pool is left as it is; it only serves as the fallback when the library's pool cannot be created.
 struct AsyncTmp {
     cudaStream_t st;
+    cudaMemPool_t pool;
     std::vector<void *> ptrs;
-    explicit AsyncTmp(cudaStream_t s) : st(s)
+    static cudaMemPool_t pool_of_current_device()
     {
-        static bool pool_configured[64] = {false};
-        int dev = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < 64 && !pool_configured[dev]) {
-            cudaMemPool_t pool;
-            if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-                uint64_t keep = UINT64_MAX;
-                cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-            }
-            pool_configured[dev] = true;
-        }
+        constexpr int MAXDEV = 64;
+        static std::once_flag once[MAXDEV];
+        static cudaMemPool_t pools[MAXDEV];
+        int dev = -1;
+        if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= MAXDEV) { cudaGetLastError(); return nullptr; }
+        std::call_once(once[dev], [dev] {
+            cudaMemPoolProps props;
+            memset(&props, 0, sizeof(props));
+            props.allocType = cudaMemAllocationTypePinned;
+            props.handleTypes = cudaMemHandleTypeNone;
+            props.location.type = cudaMemLocationTypeDevice;
+            props.location.id = dev;
+            cudaMemPool_t p = nullptr;
+            if (cudaMemPoolCreate(&p, &props) != cudaSuccess) { cudaGetLastError(); pools[dev] = nullptr; return; }
+            uint64_t keep = UINT64_MAX;
+            cudaMemPoolSetAttribute(p, cudaMemPoolAttrReleaseThreshold, &keep);
+            pools[dev] = p;
+        });
+        return pools[dev];
     }
+    explicit AsyncTmp(cudaStream_t s) : st(s), pool(pool_of_current_device()) {}
     ~AsyncTmp() { for (void *p : ptrs) cudaFreeAsync(p, st); }
     int alloc(size_t bytes, void **d)
     {
-        CUDA_TRY(cudaMallocAsync(d, bytes ? bytes : 16, st));
+        if (pool) CUDA_TRY(cudaMallocFromPoolAsync(d, bytes ? bytes : 16, pool, st));
+        else CUDA_TRY(cudaMallocAsync(d, bytes ? bytes : 16, st));
         ptrs.push_back(*d);
         return KG_OK;
     }

@@ -199,7 +199,10 @@ __global__ void __launch_bounds__(TB_THREADS, 1) kg_tb2_kernel(const Tb2Args a)
             const int nown = (int)(left < CS ? left : CS);
             const int n1 = cur_info.x, n2 = cur_info.y;
             const int nh = NSTEP == 2 ? n1 + n2 : n1;
-            const int nrow = NSTEP == 2 ? CS + ((n1 + 1) & ~1) : ((nown + 1) & ~1);
+            // always all CS own rows: the plan zero-fills the rows behind a ragged last tile (slot 0, dictionary
+            // id 0), so threads with row >= nown gather inside the stage instead of decoding what an earlier
+            // tile left there
+            const int nrow = NSTEP == 2 ? CS + ((n1 + 1) & ~1) : CS;
             const uint32_t vb = (uint32_t)nown * C * 16u;
             const uint32_t hb = (uint32_t)((nh + 3) & ~3) * 4u;
             const uint32_t rb = (uint32_t)nrow * KP * 2u;
