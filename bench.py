@@ -309,15 +309,19 @@ def run_b200(args, cfg):
     mu_avg = ctx.mean_over_ranks(mu_dos.mean(dim=0))
     mu0 = complex(mu_avg[0].item())
 
-    # dominant kernel (about 60 % of the step, profiles/): the VAC moment sweep on the batch
-    # [V psi_k | chi_k] (C = 2R columns, rows k >= 1) with the two cross inner products per Chebyshev step.
-    # On this config it is the TWO-STEP kernel kg_tb2_kernel<C, K, MODE_MOMX> (T_m+1 and T_m+2 per pass, tile +
-    # two halo rings in shared memory).  One more time step of kg_vac = velocity + column copy + [first step +
-    # ceil((M/2 - 1)/2) passes + reduction] + one evolution of the 2R-column batch, so the moment loop is timed as
-    # kg_vac(n_steps = 2) - kg_vac(n_steps = 1) - kg_evolve(2R columns), all live CUDA events on the launching
-    # stream; the launch counter says which path ran.
+    # The two moment kernels of the step, each timed as a DIFFERENCE OF TWO SERIES LENGTHS of the same call, so
+    # that everything that does not scale with M cancels exactly — first step, final reduction, velocity, column
+    # copies (including the re-layout copies of the column-pair planes on wider batches), the evolution — and
+    # only pass launches remain, counted by the library's launch counter over the same two calls:
+    #   one-column form (DOS, MSD rows, VAC row 0; MODE_MOM2 on R columns):  kg_dos_moments(M) - kg_dos_moments(M1)
+    #   cross form (VAC rows k >= 1; MODE_MOMX on the batch [V psi_k | chi_k], 2R columns):
+    #       [kg_vac(n_steps = 2, M) - kg_vac(1, M)] - [kg_vac(2, M1) - kg_vac(1, M1)]
+    # All live CUDA events on the launching stream.  On the roofline config the passes are the TWO-STEP kernel
+    # kg_tb2_kernel (T_m+1 and T_m+2 per pass, tile + two halo rings in shared memory); d(launches) against
+    # d(Chebyshev steps) says which kernel ran.
     reps = 3
     C = 2 * R
+    M1 = max(8, (M // 2) & ~3)
 
     def timed_calls(fn):
         fn(); torch.cuda.synchronize()
@@ -330,75 +334,99 @@ def run_b200(args, cfg):
         torch.cuda.synchronize()
         return e0.elapsed_time(e1) * 1e3 / reps, (h.launch_count - l0) // reps
 
-    mu_v = [torch.empty((R, k + 1, M), dtype=torch.complex128, device="cuda") for k in (1, 2)]
-    phi_c = torch.from_numpy(W.random_phase_vectors(n, C, cfg.seed)).cuda()
-    evo_out = torch.empty_like(phi_c)
-    us_v1, l_v1 = timed_calls(lambda: B.vac(h, phi_dev, M, 1, cfg.dt_fs, mu=mu_v[0]))
-    us_v2, l_v2 = timed_calls(lambda: B.vac(h, phi_dev, M, 2, cfg.dt_fs, mu=mu_v[1]))
-    us_ev, l_ev = timed_calls(lambda: B.evolve(h, phi_c, -cfg.dt_fs, out=evo_out))
-    # (kg_evolve on caller-order vectors adds two row permutations to the 41 sweeps of the evolution inside
-    # kg_vac: 2 launches and 60 us in 85 ms, i.e. the pass time below is under-estimated by < 0.1 %)
-    sweeps = (l_v2 - l_v1) - (l_ev - 2) - 4              # minus velocity, column copy, first step, reduction
-    steps = M // 2 - 1                                   # Chebyshev steps those launches perform
-    two_step = sweeps < steps
-    kern_us = (us_v2 - us_v1 - us_ev) / (sweeps + 1)     # the first step is a sweep of the same size
-    del mu_v, phi_c, evo_out
+    def vac_step(m):
+        """time and launches of ONE more time step of kg_vac at series length m"""
+        mu_v = [torch.empty((R, k + 1, m), dtype=torch.complex128, device="cuda") for k in (1, 2)]
+        us1, l1 = timed_calls(lambda: B.vac(h, phi_dev, m, 1, cfg.dt_fs, mu=mu_v[0]))
+        us2, l2 = timed_calls(lambda: B.vac(h, phi_dev, m, 2, cfg.dt_fs, mu=mu_v[1]))
+        return us2 - us1, l2 - l1
+
+    def dos_call(m):
+        mu = torch.empty((R, m), dtype=torch.complex128, device="cuda")
+        return timed_calls(lambda: B.dos_moments(h, phi_dev, m, mu=mu))
+
+    dsteps = M // 2 - M1 // 2                            # Chebyshev steps between the two series lengths (doubling)
+    (us_a, l_a), (us_b, l_b) = vac_step(M), vac_step(M1)
+    momx_t = (us_a - us_b, l_a - l_b)
+    (us_a, l_a), (us_b, l_b) = dos_call(M), dos_call(M1)
+    mom2_t = (us_a - us_b, l_a - l_b)
     peak, peak_src = peaks()
     ons = lat.onsite is not None
 
-    def kernel_block(mode, cols, us, nsweeps):
-        """roofline entry of one moment kernel: `nsweeps` launches perform `steps` Chebyshev steps on `cols` columns"""
-        two = nsweeps < steps
-        if nsweeps == 1 and steps > 2:
+    def kernel_block(mode, cols, d_us, d_launches):
+        """roofline entry of one moment kernel: `d_launches` more launches performed `dsteps` more Chebyshev
+        steps on `cols` columns in `d_us` more microseconds"""
+        one_launch = d_launches <= 0                     # the whole loop is one cluster launch: no per-pass launches to count
+        nl = 1 if one_launch else d_launches
+        spl = dsteps / nl                                # Chebyshev steps per launch
+        us = d_us / nl
+        two = (not one_launch) and spl > 1.5
+        if one_launch:
             kname = "kg_small_kernel (launch-bound size: all Chebyshev steps after the first in ONE cluster launch, vectors in distributed shared memory)"
         elif two:
-            kname = (f"kg_tb2_kernel<C={cols}, K={lat.kmax}, {mode}, NSTEP=2> (two Chebyshev steps per pass: tile + two halo rings in "
-                     "shared memory, TMA-staged streams, four inner products per pass)")
+            kname = (f"kg_tb2_kernel<C={min(cols, 2)}, K={lat.kmax}, {mode}, NSTEP=2> (two Chebyshev steps per pass: tile + two halo rings in "
+                     "shared memory, TMA-staged streams, four inner products per pass"
+                     + (f"; the {cols} columns as {cols // 2} column-pair planes side by side in one launch)" if cols > 2 else ")"))
         else:
             kname = (f"kg_staged_kernel<R={cols}, {mode}> (fused T_m+1 = 2H~T_m - T_m-1 + two inner products; TMA-staged streams, "
                      "hopping dictionary, alternating sweep)")
         if two:
             # must-move bytes of a two-step pass, per site: T_m, T_m-1 read and T_m+1, T_m+2 written (64 B per
-            # column), 8 B of tile-local matrix row (4 x uint16), 8 B on-site energy; halo re-reads not counted
-            bl = (64.0 * cols + 8.0 + (8.0 if ons else 0.0)) * n
-            bdef = ("must-move bytes of the launched two-step pass: (64 C + 8 + 8) B per site (T_m, T_m-1 read, T_m+1, T_m+2 written "
-                    "for C columns; tile-local matrix row; on-site energy), no halo, no cache reuse between launches")
+            # column), 8 B of tile-local matrix row (4 x uint16) per plane of <= 2 columns, 8 B on-site energy per
+            # plane; halo re-reads not counted
+            planes = max(1, cols // 2)
+            bl = (64.0 * cols + planes * (8.0 + (8.0 if ons else 0.0))) * n
+            bdef = ("must-move bytes of the launched two-step pass: (64 C + 8 + 8) B per site and column-pair plane (T_m, T_m-1 read, "
+                    "T_m+1, T_m+2 written for C columns; tile-local matrix row; on-site energy), no halo, no cache reuse between launches")
             tkey = f"{cfg.name}_tb2_{'momx' if mode == 'MODE_MOMX' else 'mom2'}_C{cols}"
         else:
-            bl = must_move_bytes_per_update(cols, lat.kmax, ons) * n * cols
+            bl = must_move_bytes_per_update(cols, lat.kmax, ons) * n * cols * (spl if one_launch else 1.0)
             bdef = ("must-move bytes of the launched one-step sweep: (48 + (4 K + 8)/C) B per site-update (T_m, T_m-1 read, T_m+1 "
-                    "written, packed index + on-site row shared by the C columns)")
+                    "written, packed index + on-site row shared by the C columns)"
+                    + (" times the steps of the one launch (which keeps them in shared memory: not an HBM figure)" if one_launch else ""))
             tkey = f"{cfg.name}_{'momx' if mode == 'MODE_MOMX' else 'mom2'}_R{cols}"
-        spl = steps / nsweeps if nsweeps > 0 else 1.0
         upd = n * cols * spl
         b8d = mom_bytes_per_update(cols, lat.kmax, phi_l_stream=False) * upd
         ach = bl / (us * 1e-6) / 1e9
         blk = {"bound": "hbm", "kernel": kname, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                "peak_source": peak_src, "frac_of_nominal_8TBs": ach / 8000.0, "bytes_per_launch": bl, "bytes_definition": bdef,
                "chebyshev_steps_per_launch": spl,
+               "timed_as": f"difference of the same call at M = {M} and M = {M1}: {d_launches} launches, {dsteps} Chebyshev steps, {d_us:.1f} us",
                "survey_8d_general_ell": {"bytes_per_launch": b8d, "achieved": b8d / (us * 1e-6) / 1e9, "frac": b8d / (us * 1e-6) / 1e9 / peak,
                                          "note": "SURVEY 8(d) doubling row, 48 + (12 K + 8)/C B per site-update of a one-step sweep "
                                                  "with fp64 hoppings streamed, times the site-updates one launch performs; the launched "
                                                  "kernel moves far fewer bytes (two steps per pass, hopping dictionary), so this "
                                                  "fraction exceeds 1 - the roofline fraction is `frac`, on the bytes really required"},
                "us_per_launch": us, "gsu_per_s": upd / (us * 1e-6) / 1e9, "traffic": ncu_traffic(tkey)}
-        if blk["frac"] > 1.0:
+        if 48.0 * n * cols <= 126e6:
+            blk["l2_resident"] = (f"T_m, T_m-1 and T_m+1 of the {cols} columns are {48.0 * n * cols / 1e6:.0f} MB and stay in the 126 MB L2 "
+                                  "from launch to launch: this launch is not HBM-bound and `frac` is not a roofline fraction")
+        elif blk["frac"] > 1.0:
             blk["warning"] = "frac > 1 against must-move bytes: the timed launches are not the kernel named here"
         return blk
 
-    momx = kernel_block("MODE_MOMX", C, kern_us, sweeps)
-    # the DOS / MSD / VAC-row-0 moment sweep on R columns: kg_dos_moments(M) = first step + passes + reduction
-    us_d, l_d = timed_calls(lambda: B.dos_moments(h, phi_dev, M, mu=mu_dos))
-    sweeps1 = l_d - 2                                           # minus first step, reduction
-    mom2 = kernel_block("MODE_MOM2", R, us_d / (sweeps1 + 1), sweeps1)
-    # which of the two dominates the step: launches per bench step x time per launch
-    t_momx = nt * (sweeps + 1) * momx["us_per_launch"]                  # VAC rows k = 1 .. nt
-    t_mom2 = (2 + nt) * (sweeps1 + 1) * mom2["us_per_launch"]           # DOS, VAC row 0, MSD rows 1 .. nt
+    momx = kernel_block("MODE_MOMX", C, *momx_t)
+    mom2 = kernel_block("MODE_MOM2", R, *mom2_t)
+    # which of the two dominates: passes of a moment set of M moments x time per pass (the first step and the
+    # reduction of every set are left out of the shares)
+    sets_us = {"momx": (M // 2 - 1) / momx["chebyshev_steps_per_launch"] * momx["us_per_launch"],
+               "mom2": (M // 2 - 1) / mom2["chebyshev_steps_per_launch"] * mom2["us_per_launch"]}
+    t_momx = nt * sets_us["momx"]                                        # VAC rows k = 1 .. nt
+    t_mom2 = (2 + nt) * sets_us["mom2"]                                  # DOS, VAC row 0, MSD rows 1 .. nt
     step_us = ms / args.steps * 1e3
     momx["share_of_step"] = t_momx / step_us
     mom2["share_of_step"] = t_mom2 / step_us
     roofline, other = (mom2, momx) if t_mom2 >= t_momx else (momx, mom2)
     roofline["second_kernel"] = other
+    # the bench step runs T = --time-steps of the config's N_t time steps, which over-weights the one-column form
+    # (DOS and VAC row 0 are once per job): the same two measured kernels weighted by the pass counts of the FULL
+    # job, DOS + kg_vac(N_t) + kg_msd(N_t)
+    jt_momx, jt_mom2 = cfg.n_steps * sets_us["momx"], (2 + cfg.n_steps) * sets_us["mom2"]
+    roofline["job_weighted"] = {
+        "n_steps": cfg.n_steps, "frac": (jt_momx * momx["frac"] + jt_mom2 * mom2["frac"]) / (jt_momx + jt_mom2),
+        "moment_time_share": {"MODE_MOMX": jt_momx / (jt_momx + jt_mom2), "MODE_MOM2": jt_mom2 / (jt_momx + jt_mom2)},
+        "note": "time-weighted mean of the two kernels' roofline fractions over the moment passes of the config's full job "
+                "(= their must-move bytes / their time / peak); evolutions not included"}
 
     if rank != 0:
         ctx.finalize()

@@ -46,6 +46,7 @@ def test_bench_line_on_small_config():
     assert b["e2e"]["h2d_bytes_per_step"] > 0 and b["e2e"]["d2h_bytes_per_step"] > 0
     r = b["roofline"]
     assert r["bound"] == "hbm" and r["unit"] == "GB/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
+    assert 0 < r["job_weighted"]["frac"] and "timed_as" in r and "second_kernel" in r
 
 
 def test_reference_arm_line_on_the_cpu():
