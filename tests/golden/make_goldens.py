@@ -19,14 +19,25 @@ for (only the Jackson damping does), so the oracle runs ALL time steps of each c
 per random vector.  tests/test_gpu_goldens.py runs the FULL GPU jobs and compares every stored entry.
 
 config | lattice                                   | vectors | M    | N_t | M'
-   2   | 250x250 cells, 0.5 % vacancies (seed 1)   | 0, 3    | 1000 | 200 | 64
+   2   | 250x250 cells, 0.5 % vacancies (seed 1)   | 0, 2, 3 | 1000 | 200 | 64
    3   | AGNR 15 x 20000 cells                     | 0       | 2000 | 400 | 64
    4   | 1000x1000 cells, Anderson W=|t| (seed 2)  | 0       | 3000 | 100 | 64
-   5   | 2000x2000 cells, 0.1 % vacancies (seed 3) | 0, 7    | 3000 |  50 | 16
+   5   | 2000x2000 cells, 0.1 % vacancies (seed 3) | 0,3,4,7 | 3000 |  50 | 16
    6   | ZGNR 65536 x 16 (the paper's Fig. 4)      | 0       | 2000 | 400 | 64
 
+(Config 5's vectors 3 and 4 sit in the two middle column-pair planes of the GPU's wide-batch path, one in
+each column position; 0 and 7 in the outer planes.)
+
 Every file records the sha256 of oracle/kgo.c, the git commit of the tree that wrote it, the config
-parameters and the sha256 of the random vector's bytes.  Host time on 8 cores: about 1.5 h.
+parameters and the sha256 of the random vector's bytes.  Files written from round 3 on also record
+`oracle_arith_sha256`, the sha256 of kgo.c from `kgo_bond_dx` to the end of the file — everything the
+stored numbers are computed by (operators, recursions, Bessel series, drivers), without the lattice /
+random-number generators above it, which tests/test_generators.py pins bit for bit on their own.  For the
+files written before that, `--record-versions` recomputes the same hash from the recorded git commit and
+writes tests/golden/oracle_versions.txt (`file sha256, arithmetic sha256, commit` per kgo.c version that
+wrote a stored file).  tests/test_golden_files.py compares these with today's kgo.c: a change to the
+oracle's arithmetic after a file was written fails there until the file is regenerated.
+Host time on 8 cores: about 2.5 h.
 """
 from __future__ import annotations
 
@@ -49,10 +60,10 @@ HBAR = 0.6582119569         # eV fs
 
 # name: (vectors, M, N_t, dt in units of hbar/|t|, M', wants)
 CONFIGS = {
-    2: dict(vectors=(0, 3), M=1000, nt=200, dt_mult=2, Mp=64, seed=1, wants=("dos", "vac", "msd")),
+    2: dict(vectors=(0, 2, 3), M=1000, nt=200, dt_mult=2, Mp=64, seed=1, wants=("dos", "vac", "msd")),
     3: dict(vectors=(0,), M=2000, nt=400, dt_mult=1, Mp=64, seed=0, wants=("dos", "msd")),
     4: dict(vectors=(0,), M=3000, nt=100, dt_mult=4, Mp=64, seed=2, wants=("dos", "vac", "msd")),
-    5: dict(vectors=(0, 7), M=3000, nt=50, dt_mult=8, Mp=16, seed=3, wants=("dos", "msd")),
+    5: dict(vectors=(0, 3, 4, 7), M=3000, nt=50, dt_mult=8, Mp=16, seed=3, wants=("dos", "msd")),
     6: dict(vectors=(0,), M=2000, nt=400, dt_mult=1, Mp=64, seed=0, wants=("dos", "msd")),
 }
 
@@ -113,15 +124,47 @@ def cost(piece):
     return n * (c["nt"] * per_step + 2 * c["M"])
 
 
+ARITH_START = b"static double kgo_bond_dx"      # first function of kgo.c after the generators
+
+
+def arith_sha256(src: bytes) -> str:
+    """sha256 of kgo.c from its first operator function to the end (see the module docstring)."""
+    return hashlib.sha256(src[src.index(ARITH_START):]).hexdigest()
+
+
 def provenance():
     with open(os.path.join(ROOT, "oracle", "kgo.c"), "rb") as f:
-        osha = hashlib.sha256(f.read()).hexdigest()
+        src = f.read()
+    osha = hashlib.sha256(src).hexdigest()
     try:
         commit = subprocess.run(["git", "-C", ROOT, "rev-parse", "HEAD"], capture_output=True, text=True,
                                 check=True).stdout.strip()
     except Exception:
         commit = "unknown"
-    return osha, commit
+    return osha, arith_sha256(src), commit
+
+
+def record_versions(outdir):
+    """tests/golden/oracle_versions.txt: for every (kgo.c sha256, git commit) recorded in a stored file,
+    the arithmetic hash of kgo.c AS IT WAS at that commit (read with `git show`)."""
+    import ast
+    seen = {}
+    for name in sorted(os.listdir(outdir)):
+        if name.endswith(".npz"):
+            meta = ast.literal_eval(str(np.load(os.path.join(outdir, name))["meta"]))
+            seen[meta["oracle_kgo_c_sha256"]] = meta["git_commit"]
+    lines = ["# kgo.c versions that wrote the stored oracle outputs: file sha256, sha256 from kgo_bond_dx to the end, commit",
+             "# written by tests/golden/make_goldens.py --record-versions (git show <commit>:oracle/kgo.c)"]
+    for osha, commit in sorted(seen.items(), key=lambda kv: kv[1]):
+        src = subprocess.run(["git", "-C", ROOT, "show", f"{commit}:oracle/kgo.c"], capture_output=True, check=True).stdout
+        if hashlib.sha256(src).hexdigest() != osha:      # written from a tree with uncommitted changes to kgo.c
+            with open(os.path.join(ROOT, "oracle", "kgo.c"), "rb") as f:
+                src = f.read()
+            assert hashlib.sha256(src).hexdigest() == osha, f"kgo.c with sha256 {osha} is neither at {commit} nor in the tree"
+        lines.append(f"{osha} {arith_sha256(src)} {commit}")
+    with open(os.path.join(outdir, "oracle_versions.txt"), "w") as f:
+        f.write("\n".join(lines) + "\n")
+    print("\n".join(lines))
 
 
 def run_piece(piece, outdir, shrink=1, nt_override=None):
@@ -136,9 +179,9 @@ def run_piece(piece, outdir, shrink=1, nt_override=None):
     M, Mp = c["M"], c["Mp"]
     nt = c["nt"] if nt_override is None else nt_override
     dt = c["dt_mult"] * HBAR / T
-    osha, commit = provenance()
+    osha, asha, commit = provenance()
     meta = dict(config=idx, vector=r, n=lat.n, M=M, Mp=Mp, nt=nt, dt_fs=dt, scale=s, e0=0.0, seed=c["seed"],
-                shrink=shrink, phi_sha256=hashlib.sha256(phi.tobytes()).hexdigest(), oracle_kgo_c_sha256=osha,
+                shrink=shrink, phi_sha256=hashlib.sha256(phi.tobytes()).hexdigest(), oracle_kgo_c_sha256=osha, oracle_arith_sha256=asha,
                 git_commit=commit, written_by="tests/golden/make_goldens.py")
     arrays = {}
     if job == "dos":
@@ -171,7 +214,11 @@ def main():
     ap.add_argument("--shrink", type=int, default=1, help="debug: divide the linear size of the lattices")
     ap.add_argument("--time-steps", type=int, default=None, help="debug: override N_t")
     ap.add_argument("--skip-existing", action="store_true")
+    ap.add_argument("--record-versions", action="store_true", help="write oracle_versions.txt from the stored files and git")
     args = ap.parse_args()
+    if args.record_versions:
+        record_versions(args.out)
+        return
     if args.piece:
         run_piece(args.piece, args.out, args.shrink, args.time_steps)
         return

@@ -5,6 +5,7 @@ for bit the head of the full row stored for that step (moments do not depend on 
 for), mu_0 = 1 for the unit-norm vector, |mu_m| <= 1, the DOS moments are real, MSD starts from 0 and
 its zeroth moment ||psix_k||^2 grows."""
 import ast
+import hashlib
 import os
 
 import numpy as np
@@ -21,6 +22,39 @@ SHAPES = {2: (248750, 1000, 200, 64), 3: (1200000, 2000, 400, 64), 4: (4000000, 
 def load(name):
     d = np.load(os.path.join(GOLDEN, name + ".npz"))
     return d, ast.literal_eval(str(d["meta"]))
+
+
+def _arith_sha256_today():
+    """sha256 of oracle/kgo.c from its first operator function to the end: everything the stored numbers are
+    computed by (the generators above it are pinned bit for bit by tests/test_generators.py)."""
+    src = open(os.path.join(os.path.dirname(GOLDEN), os.pardir, "oracle", "kgo.c"), "rb").read()
+    return hashlib.sha256(src[src.index(b"static double kgo_bond_dx"):]).hexdigest()
+
+
+def _recorded_versions():
+    """tests/golden/oracle_versions.txt: file sha256 -> arithmetic sha256 of the kgo.c versions that wrote files
+    before the files recorded the arithmetic hash themselves (make_goldens.py --record-versions)."""
+    table = {}
+    with open(os.path.join(GOLDEN, "oracle_versions.txt")) as f:
+        for line in f:
+            w = line.split("#")[0].split()
+            if len(w) >= 2:
+                table[w[0]] = w[1]
+    return table
+
+
+def test_stored_outputs_were_written_by_todays_oracle_arithmetic():
+    """Every stored file was written by a kgo.c whose operators, recursions, series and drivers are byte for
+    byte today's: if the oracle's arithmetic is changed after a file was written this fails until the file is
+    regenerated, so the GPU is never compared with numbers the current oracle would not produce."""
+    today, table = _arith_sha256_today(), _recorded_versions()
+    files = sorted(f for f in os.listdir(GOLDEN) if f.endswith(".npz"))
+    assert len(files) >= 17
+    for name in files:
+        meta = ast.literal_eval(str(np.load(os.path.join(GOLDEN, name))["meta"]))
+        wrote = meta.get("oracle_arith_sha256") or table.get(meta["oracle_kgo_c_sha256"])
+        assert wrote is not None, f"{name}: kgo.c version {meta['oracle_kgo_c_sha256'][:12]} is not in oracle_versions.txt"
+        assert wrote == today, f"{name} was written by a different oracle arithmetic: regenerate it (make_goldens.py --piece {name[:-4]})"
 
 
 @pytest.mark.parametrize("idx", [2, 3, 4, 5, 6])

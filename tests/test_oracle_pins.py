@@ -316,6 +316,52 @@ def test_msd_vs_dense(kgo):
     assert np.max(np.abs(got.imag)) < 1e-12 * np.max(np.abs(got))
 
 
+def test_vac_msd_ragged_schedule_vs_dense(kgo):
+    """The branch of the VAC / MSD drivers that every stored output under tests/golden/ goes through
+    (tests/golden/make_goldens.py): kgo_vac_sched / kgo_msd_sched with a NON-constant number of moments per
+    time step — rows shorter than the row stride, and a row with no moments at all, where the states are
+    only advanced.  Pinned (a) directly on the dense formulas, eq 33 and eq 34 + eq 44 composition,
+    row by row at the scheduled lengths — so a wrong row stride, a row written to the wrong place or an
+    evolution dropped on the skipped row fails here without reference to any other oracle routine; (b) on
+    the constant-schedule drivers: a Chebyshev moment does not depend on how many are asked for, so every
+    scheduled row is bit for bit the head of the full row; (c) entries behind a row's length stay 0."""
+    lat = small_disordered(kgo, open_x=True)
+    H, E, Vec = eig(lat)
+    s = (3 * 2.7 + 1.35) * 1.05
+    X = np.diag(lat.x)
+    V = (1j / HBAR) * (H @ X - X @ H)
+    phi = rand_state(lat.n, 21)
+    dt = 0.7
+    Mk = np.array([24, 5, 0, 7, 24], np.int32)
+    nt, ld = len(Mk) - 1, int(Mk.max())
+    Tn = [dense_Tn(E, Vec, m, 0.0, s) for m in range(ld)]
+    got_v = kgo.vac_sched(lat, lat.x, 0.0, 0.0, s, phi, Mk, dt)
+    got_m = kgo.msd_sched(lat, lat.x, 0.0, 0.0, s, phi, Mk, dt)
+    assert got_v.shape == (nt + 1, ld) and got_m.shape == (nt + 1, ld)
+    full_v = kgo.vac(lat, lat.x, 0.0, 0.0, s, phi, ld, nt, dt)
+    full_m = kgo.msd(lat, lat.x, 0.0, 0.0, s, phi, ld, nt, dt)
+    for k in range(nt + 1):
+        Ud = dense_U(E, Vec, -k * dt)
+        L, R = V @ (Ud @ phi), Ud @ (V @ phi)
+        U = dense_U(E, Vec, k * dt)
+        px = (X @ U - U @ X) @ phi
+        want_v = np.array([np.vdot(L, Tn[m] @ R) for m in range(Mk[k])])
+        want_m = np.array([np.vdot(px, Tn[m] @ px) for m in range(Mk[k])])
+        if Mk[k]:
+            assert relerr(got_v[k, :Mk[k]], want_v) < 1e-12, k                       # (a)
+            if k:
+                assert relerr(got_m[k, :Mk[k]], want_m) < 1e-12, k
+        assert got_v[k, :Mk[k]].tobytes() == full_v[k, :Mk[k]].tobytes(), k          # (b)
+        assert got_m[k, :Mk[k]].tobytes() == full_m[k, :Mk[k]].tobytes(), k
+        assert np.all(got_v[k, Mk[k]:] == 0) and np.all(got_m[k, Mk[k]:] == 0)       # (c)
+    assert np.all(got_m[0] == 0)
+    # a schedule that skips the FIRST row and keeps one moment on the last (row stride 1)
+    one = kgo.vac_sched(lat, lat.x, 0.0, 0.0, s, phi, np.array([0, 0, 1], np.int32), dt)
+    assert one.shape == (3, 1) and one[0, 0] == 0 and one[1, 0] == 0
+    Ud = dense_U(E, Vec, -2 * dt)
+    assert abs(one[2, 0] - np.vdot(V @ (Ud @ phi), Ud @ (V @ phi))) < 1e-12 * abs(one[2, 0])
+
+
 def test_ring_vac_constant_msd_quadratic(kgo):
     """1-D ring: [V,H] = 0 => mu^VAC_n(t) independent of t and mu^MSD_n(t) = t^2 <V phi|T_n|V phi>
     per vector, exactly."""
