@@ -6,7 +6,8 @@ For the chosen config (1..5, `workloads.make_config`) this computes what BASELIN
 outputs — DOS moments, VAC and/or MSD moments over all its correlation-time steps — then, still
 on the device, the KPM reconstructions on the config's energy grid (eqs 29-31, 35), the running
 conductivities sigma_GK / sigma_E1 / sigma_E2 in e^2/h (eqs 6, 9, 11) and, for the ribbon, the
-ballistic conductance (eqs 50-51).  It prints one JSON line with timings and a few physical
+ballistic conductance (eqs 50-51).  It prints one JSON line with timings (`setup_s` = synthetic lattice and vectors generated with numpy on the
+host + `create_s`, the kg_create_hamiltonian call alone) and a few physical
 sanity numbers (integral of the DOS, Einstein vs Green-Kubo agreement, conductance near the band
 centre) and, with --out, saves the arrays as a compressed .npz.
 
@@ -52,7 +53,10 @@ def main(argv=None):
     n, R = lat.n, cfg.R
     M = args.moments or cfg.M
     nt = cfg.n_steps if args.time_steps is None else args.time_steps
-    h = B.from_lattice(lat, cfg.xcoord, cfg.period, cfg.e0, cfg.scale)
+    torch.cuda.synchronize()
+    t_create = time.perf_counter()
+    h = B.from_lattice(lat, cfg.xcoord, cfg.period, cfg.e0, cfg.scale)        # synchronises (validation result)
+    t_create = time.perf_counter() - t_create
     phi = torch.from_numpy(W.random_phase_vectors(n, R, cfg.seed)).cuda()
     energies = torch.from_numpy(W.energy_grid(cfg.n_energies)).cuda()
     t_setup = time.perf_counter() - t0
@@ -117,7 +121,7 @@ def main(argv=None):
     en = energies.cpu().numpy()
 
     summary = {"config": cfg.name, "sites": n, "R": R, "M": M, "time_steps": nt, "dt_fs": cfg.dt_fs,
-               "setup_s": round(t_setup, 3), **{k: (round(v, 4) if isinstance(v, float) else v) for k, v in timing.items()},
+               "setup_s": round(t_setup, 3), "create_s": round(t_create, 3), **{k: (round(v, 4) if isinstance(v, float) else v) for k, v in timing.items()},
                "workspace_GB": round(h.workspace_bytes / 1e9, 3)}
     sweeps = timing["dos_launches"] + timing.get("vac_launches", 0) + timing.get("msd_launches", 0)
     summary["kernel_launches"] = int(sweeps)

@@ -47,6 +47,7 @@ def test_bench_line_on_small_config():
     r = b["roofline"]
     assert r["bound"] == "hbm" and r["unit"] == "GB/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
     assert 0 < r["job_weighted"]["frac"] and "timed_as" in r and "second_kernel" in r
+    assert b["setup"]["create_s"] > 0 and b["setup"]["first_step_s"] > 0
 
 
 def test_reference_arm_line_on_the_cpu():
