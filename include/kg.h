@@ -34,8 +34,9 @@
  *
  * STREAMS.  `stream` is a cudaStream_t cast to void* (NULL = legacy default stream).  Calls
  * enqueue work on it and return without synchronising, except: kg_create_hamiltonian[_csr]
- * (validation result), the first moments call of a handle that builds the two-step kernel's
- * tile plan (KG_OPT_TWO_STEP), calls that have to grow the workspace while a cached CUDA graph
+ * (validation result; also builds the two-step kernel's tile plans where KG_OPT_TWO_STEP's
+ * default will use them), the first moments call after KG_OPT_TWO_STEP was forced on a handle
+ * whose plan create did not build, calls that have to grow the workspace while a cached CUDA graph
  * refers to it, calls with KG_OPT_CHECK_INPUT set, and calls whose outputs are pageable host
  * memory.  Device outputs are valid once the stream has been synchronised.
  *

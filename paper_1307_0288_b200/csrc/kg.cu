@@ -380,7 +380,8 @@ __global__ void kg_tb2_gather_onsite(const double *__restrict__ onsite, const in
 }
 
 // Build the per-tile plan for C columns per site from the packed list (dictionary id << 28 | index,
-// internal order).  Runs once per handle and C, at the first eligible moments call; synchronises.
+// internal order).  Runs once per handle and C — at create for the handles the automatic choice serves, else at
+// the first eligible moments call; synchronises.
 static int tb2_build_plan(kg_hamiltonian *h, int C, cudaStream_t st)
 {
     Tb2Plan &tp = h->tbp[C - 1];
@@ -708,6 +709,20 @@ static int create_from_device_list(kg_hamiltonian **out, int64_t n, int kmax, co
         cudaFree(d_tab); cudaFree(d_dict);
     }
     cudaFree(d_flags);
+    d_flags = nullptr;
+    // Tile plans of the two-step kernel for the handles on which the automatic choice (tb2_plan) will use it —
+    // re-ordered sites, at least four tiles per SM — are built here, so that no moments call has to stop and
+    // synchronise for them.  (A handle on which KG_OPT_TWO_STEP is forced later builds its plan at the first
+    // moments call, as before.)
+    if (h->perm) try {
+        for (int C = 1; C <= 2; ++C) {
+            const int64_t nt = (n + tb_cs(C) - 1) / tb_cs(C);
+            if (nt < 4 * (int64_t)h->num_sms) continue;
+            if ((rc = tb2_build_plan(h, C, st))) return cleanup(rc);
+        }
+    } catch (const std::bad_alloc &) {
+        return cleanup(fail(KG_ENOMEM, "host allocation failed in the two-step tile plan"));
+    }
     *out = h;
     return KG_OK;
 }
