@@ -14,7 +14,7 @@ import pytest
 from helpers import GOLDEN
 
 PIECES = {2: ("dos", "vac", "msd"), 3: ("dos", "msd"), 4: ("dos", "vac", "msd"), 5: ("dos", "msd"), 6: ("dos", "msd")}
-VECTORS = {2: (0, 3), 3: (0,), 4: (0,), 5: (0, 7), 6: (0,)}
+VECTORS = {2: (0, 2, 3), 3: (0,), 4: (0,), 5: (0, 3, 4, 7), 6: (0,)}
 SHAPES = {2: (248750, 1000, 200, 64), 3: (1200000, 2000, 400, 64), 4: (4000000, 3000, 100, 64),
           5: (15984000, 3000, 50, 16), 6: (1048576, 2000, 400, 64)}
 
@@ -49,7 +49,7 @@ def test_stored_outputs_were_written_by_todays_oracle_arithmetic():
     regenerated, so the GPU is never compared with numbers the current oracle would not produce."""
     today, table = _arith_sha256_today(), _recorded_versions()
     files = sorted(f for f in os.listdir(GOLDEN) if f.endswith(".npz"))
-    assert len(files) >= 17
+    assert len(files) >= 24
     for name in files:
         meta = ast.literal_eval(str(np.load(os.path.join(GOLDEN, name))["meta"]))
         wrote = meta.get("oracle_arith_sha256") or table.get(meta["oracle_kgo_c_sha256"])

@@ -62,7 +62,7 @@ def rowwise_err(got, want):
 
 # config 5 runs its 8 vectors as four column-pair planes: 0 / 7 are in the outer planes, 3 / 4 in the two middle
 # ones, and both column positions of a plane are covered
-VECTORS = {2: (0, 3), 3: (0,), 4: (0,), 5: (0, 7), 6: (0,)}
+VECTORS = {2: (0, 2, 3), 3: (0,), 4: (0,), 5: (0, 3, 4, 7), 6: (0,)}
 WANTS = {2: ("vac", "msd"), 3: ("msd",), 4: ("vac", "msd"), 5: ("msd",), 6: ("msd",)}
 
 
