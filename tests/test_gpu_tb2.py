@@ -219,3 +219,24 @@ def test_two_step_wider_batches_as_column_pair_planes(B, kgo, reordered, R):
     h.set_option(B.KG_OPT_TWO_STEP, 0)
     assert relerr(host(B.dos_moments(h, dev(phi), M)), dos) <= 1e-12
     assert relerr(host(B.vac(h, dev(phi), M, nt, dt)), vac) <= 1e-12
+
+
+def test_tile_plans_are_built_at_create_on_auto_handles(B):
+    """A handle on which the two-step kernel is chosen automatically (re-ordered sites, >= 4 tiles per SM: here
+    config 3's 1.2 M-site ribbon) gets its tile plans inside kg_create_hamiltonian, so the FIRST moments call
+    enqueues exactly the launches of the second one (the plan builder's own kernel is not among them) and is
+    bitwise equal to it; the two-step passes really run (fewer launches than Chebyshev steps)."""
+    cfg = W.make_config(3)
+    lat = cfg.lattice
+    h = B.from_lattice(lat, cfg.xcoord, cfg.period, cfg.e0, cfg.scale)
+    phi = dev(W.random_phase_vectors(lat.n, 1, cfg.seed))
+    M = 40
+    l0 = h.launch_count
+    mu1 = host(B.dos_moments(h, phi, M))
+    l1 = h.launch_count
+    mu2 = host(B.dos_moments(h, phi, M))
+    l2 = h.launch_count
+    assert l1 - l0 == l2 - l1
+    assert l2 - l1 < M // 2                        # M/2 - 1 = 19 steps in 10 passes + first step, permutation, reduction
+    assert mu1.tobytes() == mu2.tobytes()
+    assert abs(mu1[0, 0] - 1.0) < 1e-12
